@@ -1,0 +1,144 @@
+/*
+ * mlp.h -- C-ABI of the B200 (sm_100a) mini-batch SGD library for the shallow ReLU/MSE MLP
+ * of arxiv/paper_2606_30497 (32-H-1, no bias).
+ *
+ * What the library computes, per mini-batch of m rows (eqs. 1-9):
+ *   (1) Z1 = X W1   (2) H = ReLU(Z1)   (3) Ypred = H W2   (4) L = (1/m) sum (Ypred - Y)^2
+ *   (5) dZ2 = (2/m)(Ypred - Y)   (6) dW2 = H^T dZ2   (7) dZ1 = (dZ2 W2^T) (.) [Z1 > 0]
+ *   (8) dW1 = X^T dZ1            (9) W <- W - lr dW   (both matrices, after both gradients)
+ * iterated over every batch of every epoch.  ReLU'(x) = 1 if x > 0,
+ * otherwise 0.  m is the row count of the current batch (a short tail batch
+ * uses its own m).  Batches are contiguous row ranges [t*batch, min(n,(t+1)*batch)).
+ *
+ * Conventions
+ *   - Pointers named X, Y, W1, W2, batch_order, d_out are DEVICE pointers owned by the caller
+ *     (e.g. torch allocations); pointers with an `_host` suffix are HOST pointers.  The library
+ *     never frees or retains caller memory.  Library-owned scratch is created lazily and
+ *     released by mlp_shutdown().
+ *   - Layout: all tensors fp32, row-major, dense: X [n x 32], Y [n], W1 [32 x hidden],
+ *     W2 [hidden].  X must be 16-byte aligned, Y 4-byte aligned, W1 16-byte aligned.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Functions returning int return MLP_OK (0) or a positive mlp_status; nothing throws or
+ *     calls exit().  Errors detected before launch leave W1/W2 untouched.  mlp_last_error()
+ *     describes the most recent failure on the calling thread.
+ *   - One model descriptor per process (set by mlp_init); calls on different streams with
+ *     different buffers may overlap.
+ *   - There is no CPU fallback: without a CUDA device every compute entry returns MLP_ERR_CUDA.
+ */
+#ifndef PAPER_2606_30497_MLP_H
+#define PAPER_2606_30497_MLP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MLP_OK = 0,
+    MLP_ERR_NOT_INIT = 1,     /* mlp_init has not been called */
+    MLP_ERR_BAD_ARG = 2,      /* NULL pointer, n < 1, batch < 1, epochs < 0, non-finite lr, ... */
+    MLP_ERR_UNSUPPORTED = 3,  /* dimensions / variant / cluster size outside the supported set */
+    MLP_ERR_ALIGN = 4,        /* X or W1 not 16-byte aligned */
+    MLP_ERR_CUDA = 5          /* a CUDA runtime call failed (see mlp_last_error) */
+} mlp_status;
+
+/* `variant` of mlp_train_ex / mlp_eval_loss_async */
+enum {
+    MLP_VARIANT_FUSED = 0,    /* training: persistent fused cluster kernel, exact fp32 (FFMA)   */
+                              /* eval:     streaming fp32 kernel (FFMA)                          */
+    MLP_VARIANT_UNFUSED = 1,  /* training: one kernel per equation, launched per step (baseline) */
+    MLP_VARIANT_TF32 = 2      /* eval:     tcgen05 TF32 tensor-core first layer (own tolerance)  */
+};
+
+/*
+ * mlp_init -- PAPER.md:98-116.  Records the model descriptor {seed, in, hidden, out}.
+ * Supported: in == 32, out == 1, hidden in {32, 64, 128, 256, 512, 1024} (the paper's
+ * hidden-width sweep).  Anything else -> MLP_ERR_UNSUPPORTED.  No device work.
+ * May be called again to switch model.
+ */
+int mlp_init(uint64_t seed, int in, int hidden, int out);
+
+/*
+ * mlp_init_weights -- fills W1 [in*hidden] and W2 [hidden] (device) with U(+-1/sqrt(fan_in)),
+ * fan_in = in for W1 and hidden for W2 (BASELINE.json configs).  Counter-based, so a second
+ * implementation can restate it: for flat element index e (W1 row-major, then W2)
+ *     z = seed + 0x9E3779B97F4A7C15 * (e + 1)                       (mod 2^64)
+ *     z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9
+ *     z = (z ^ (z >> 27)) * 0x94D049BB133111EB
+ *     z =  z ^ (z >> 31)
+ *     u = (z >> 40) * 2^-24 ;   w = (float)((2u - 1) * bound),  bound = 1/sqrt(fan_in) in double.
+ * Asynchronous on `stream`.
+ */
+int mlp_init_weights(float* W1, float* W2, void* stream);
+
+/*
+ * mlp_train -- eqs. 1-9 over `epochs` passes of ceil(n/batch) sequential batches
+ * (PAPER.md:108-112).  Updates W1/W2 in place; X, Y read-only.  Asynchronous on `stream`
+ * (the weights are valid once the stream is synchronised).  epochs == 0 is a no-op.
+ * lr == 0 leaves the weights bit-identical.  batch > n is allowed (one short batch per epoch).
+ * Equivalent to mlp_train_ex(..., NULL, MLP_VARIANT_FUSED, stream).
+ */
+int mlp_train(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
+              float* W1, float* W2, void* stream);
+
+/*
+ * mlp_train_ex -- as mlp_train, plus
+ *   batch_order: NULL, or device int32 [epochs * nb], nb = ceil(n/batch): step e*nb+k trains on
+ *                batch index batch_order[e*nb+k] (BASELINE.json configs 2-5: "batch order a
+ *                per-epoch permutation").  Entries must lie in [0, nb); not validated on device.
+ *   variant:     MLP_VARIANT_FUSED or MLP_VARIANT_UNFUSED.
+ */
+int mlp_train_ex(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
+                 float* W1, float* W2, const int32_t* batch_order, int variant, void* stream);
+
+/*
+ * mlp_eval_loss -- eq. 4 over the whole dataset:
+ *   L = (1/n) sum_r (ReLU(X_r W1) W2 - Y_r)^2.
+ * Synchronises `stream` and returns L; NaN on error (then see mlp_last_error()).
+ * Deterministic: fp32 inside a row, fp64 from the per-warp partial upwards, fixed tree.
+ */
+double mlp_eval_loss(const float* X, const float* Y, int64_t n,
+                     const float* W1, const float* W2, void* stream);
+
+/* As mlp_eval_loss without the synchronisation: the loss is written to *d_out (device double). */
+int mlp_eval_loss_async(const float* X, const float* Y, int64_t n, const float* W1,
+                        const float* W2, double* d_out, int variant, void* stream);
+
+/*
+ * Host-buffer entry points (end-to-end path): copy X/Y (and weights / order) from HOST memory
+ * to library-owned device buffers, run the same kernels, copy the result back, synchronise.
+ * W1_host/W2_host are read and overwritten with the trained weights.  order_host may be NULL.
+ */
+int mlp_train_host(const float* X_host, const float* Y_host, int64_t n, int batch, float lr,
+                   int epochs, float* W1_host, float* W2_host, const int32_t* order_host,
+                   int variant);
+double mlp_eval_loss_host(const float* X_host, const float* Y_host, int64_t n,
+                          const float* W1_host, const float* W2_host, int variant);
+
+/*
+ * Tuning knobs of the fused training kernel.  cluster: number of CTAs (= SMs) the hidden
+ * dimension is split over; 0 = automatic.  Valid values are those with hidden/cluster in
+ * {16, 32, 64} and cluster in {1, 2, 4, 8, 16}.  Returns MLP_ERR_UNSUPPORTED otherwise.
+ */
+int mlp_set_cluster(int cluster);
+int mlp_get_cluster(void);          /* the cluster size the next mlp_train would use */
+
+/*
+ * Statistics of the most recent fused mlp_train* call that has completed (call after
+ * synchronising its stream): out[0] = SM clock cycles spent in the kernel (clock64 delta of
+ * CTA 0), out[1] = nanoseconds (globaltimer delta), out[2] = SGD steps, out[3] = cluster size.
+ */
+int mlp_get_train_stats(double out[4]);
+
+/* Number of kernels this library has launched since load (all entry points). */
+int64_t mlp_launch_count(void);
+
+const char* mlp_last_error(void);   /* static thread-local string; never NULL */
+const char* mlp_version(void);
+void mlp_shutdown(void);            /* frees library-owned device scratch; idempotent */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAPER_2606_30497_MLP_H */

@@ -1,0 +1,46 @@
+// internal.h -- declarations shared by the translation units of libmlp_b200 (host side).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mlp {
+
+constexpr int kIn = 32;   // input features
+
+// Every launcher returns cudaSuccess or the launch error and adds the kernels it launched
+// to *launches.
+
+// train_fused.cu -- persistent fused cluster kernel
+bool fused_supported(int hidden, int cluster);
+int fused_default_cluster(int hidden);
+cudaError_t launch_train_fused(const float* X, const float* Y, int64_t n, int batch, float lr,
+                               int epochs, float* W1, float* W2, const int32_t* order,
+                               int hidden, int cluster, unsigned long long* stats,
+                               cudaStream_t stream, int64_t* launches);
+
+// unfused.cu -- one kernel per equation (row a-U) + weight initialisation
+struct UnfusedScratch {
+    float *Z1, *Hact, *dZ1;   // [batch x hidden]
+    float *Ypred, *dZ2;       // [batch]
+    float *dW1, *dW2;         // [32 x hidden], [hidden]
+};
+cudaError_t launch_train_unfused(const float* X, const float* Y, int64_t n, int batch, float lr,
+                                 int epochs, float* W1, float* W2, const int32_t* order_host,
+                                 int hidden, const UnfusedScratch& s, cudaStream_t stream,
+                                 int64_t* launches);
+cudaError_t launch_init_weights(uint64_t seed, int hidden, float* W1, float* W2,
+                                cudaStream_t stream, int64_t* launches);
+
+// eval_fp32.cu -- streaming forward + MSE (row a-E)
+int eval_fp32_grid(int hidden, int num_sms);
+cudaError_t launch_eval_fp32(const float* X, const float* Y, int64_t n, const float* W1,
+                             const float* W2, int hidden, double* partials, int grid,
+                             double* d_out, cudaStream_t stream, int64_t* launches);
+
+// eval_tf32.cu -- tcgen05 TF32 first layer (row a-T, separately reported)
+bool eval_tf32_supported(int hidden);
+cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const float* W1,
+                             const float* W2, int hidden, double* partials, int grid,
+                             double* d_out, cudaStream_t stream, int64_t* launches);
+
+}  // namespace mlp

@@ -1,0 +1,247 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Run with `-m gpu` on a B200.
+
+Gate (BASELINE.json north_star; metric defined in SURVEY.md 8(c)): per matrix,
+max|gpu - oracle| / max|oracle|  <= 1e-5 after 1 step, <= 1e-3 after 1 epoch; final eval loss
+within 1 % relative.  Exact-fp32 paths are expected ~100x inside these gates.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import mlp_oracle as O                      # noqa: E402
+from paper_2606_30497_b200 import binding as B          # noqa: E402
+from paper_2606_30497_b200 import datagen               # noqa: E402
+
+LR = np.float32(0.002)
+TOL_STEP, TOL_EPOCH, TOL_LOSS = 1e-5, 1e-3, 1e-2
+
+
+def nerr(g, o):
+    g = np.asarray(g, np.float64); o = np.asarray(o, np.float64)
+    return float(np.abs(g - o).max() / max(np.abs(o).max(), 1e-30))
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_train(X, Y, W1, W2, batch, lr, epochs, order=None, variant=B.VARIANT_FUSED, cluster=0,
+              hidden=None):
+    hidden = hidden or W1.shape[1]
+    B.mlp_init(2, 32, hidden, 1)
+    B.mlp_set_cluster(cluster)
+    dX, dY, d1, d2 = dev(X), dev(Y), dev(W1), dev(W2)
+    dO = dev(order.reshape(-1)) if order is not None else None
+    B.mlp_train_ex(dX, dY, X.shape[0], batch, lr, epochs, d1, d2, dO, variant)
+    torch.cuda.synchronize()
+    B.mlp_set_cluster(0)
+    return d1.cpu().numpy(), d2.cpu().numpy()
+
+
+def gpu_eval(X, Y, W1, W2, variant=B.VARIANT_FUSED):
+    B.mlp_init(2, 32, W1.shape[1], 1)
+    dX, dY, d1, d2 = dev(X), dev(Y), dev(W1), dev(W2)
+    if variant == B.VARIANT_FUSED:
+        return B.mlp_eval_loss(dX, dY, X.shape[0], d1, d2)
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    B.mlp_eval_loss_async(dX, dY, X.shape[0], d1, d2, out, variant)
+    torch.cuda.synchronize()
+    return float(out.item())
+
+
+@pytest.fixture(scope="module")
+def cfg1():
+    X, Y = datagen.make_dataset(1024, 0.01)
+    B.mlp_init(2, 32, 256, 1)
+    d1 = torch.empty(32, 256, device="cuda"); d2 = torch.empty(256, device="cuda")
+    B.mlp_init_weights(d1, d2)
+    torch.cuda.synchronize()
+    return X, Y, d1.cpu().numpy(), d2.cpu().numpy()
+
+
+# ------------------------------------------------------------------ init
+@pytest.mark.parametrize("hidden", [32, 256, 1024])
+def test_init_weights_bit_exact(hidden):
+    B.mlp_init(2, 32, hidden, 1)
+    d1 = torch.empty(32, hidden, device="cuda"); d2 = torch.empty(hidden, device="cuda")
+    B.mlp_init_weights(d1, d2)
+    torch.cuda.synchronize()
+    o1, o2 = O.init_weights(2, 32, hidden)
+    assert d1.cpu().numpy().tobytes() == o1.tobytes()
+    assert d2.cpu().numpy().tobytes() == o2.tobytes()
+
+
+# ------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("cluster", [0, 4, 8, 16])
+def test_config1_one_step_and_epoch(cfg1, cluster):
+    X, Y, W1, W2 = cfg1
+    g1, g2 = gpu_train(X[:256], Y[:256], W1, W2, 256, LR, 1, cluster=cluster)
+    o1, o2 = O.train(X[:256], Y[:256], W1, W2, 256, LR, 1)
+    assert nerr(g1, o1) <= TOL_STEP and nerr(g2, o2) <= TOL_STEP, (nerr(g1, o1), nerr(g2, o2))
+    assert np.abs(g1 - W1).max() > 0                      # it did train
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 1, cluster=cluster)
+    o1, o2 = O.train(X, Y, W1, W2, 256, LR, 1)
+    assert nerr(g1, o1) <= TOL_EPOCH and nerr(g2, o2) <= TOL_EPOCH
+    assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5  # exact fp32 does far better than the gate
+    lg, lo = gpu_eval(X, Y, g1, g2), O.eval_loss(X, Y, o1, o2)
+    assert abs(lg - lo) <= TOL_LOSS * lo
+    assert abs(lg - lo) <= 1e-5 * lo
+
+
+def test_config1_unfused_baseline(cfg1):
+    X, Y, W1, W2 = cfg1
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 1, variant=B.VARIANT_UNFUSED)
+    o1, o2 = O.train(X, Y, W1, W2, 256, LR, 1)
+    assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5
+
+
+# ------------------------------------------------------------------ config 2 (shuffled batch order)
+def test_config2_epoch_and_final_loss():
+    c = datagen.CONFIGS["config2"]
+    X, Y = datagen.make_dataset(c.n, c.sigma)
+    W1, W2 = O.init_weights(2, 32, c.hidden)
+    order = datagen.make_order(c.n, c.batch, c.epochs, True)
+    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1])
+    o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1])
+    assert nerr(g1, o1) <= TOL_EPOCH and nerr(g2, o2) <= TOL_EPOCH, (nerr(g1, o1), nerr(g2, o2))
+    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order)
+    o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order)
+    lg, lo = gpu_eval(X, Y, g1, g2), O.eval_loss(X, Y, o1, o2)
+    assert abs(lg - lo) <= TOL_LOSS * lo, (lg, lo)
+    assert nerr(g1, o1) <= TOL_EPOCH and nerr(g2, o2) <= TOL_EPOCH
+
+
+# ------------------------------------------------------------------ config 4 shapes (hidden sweep)
+@pytest.mark.parametrize("hidden", [32, 64, 128, 512, 1024])
+def test_hidden_sweep(hidden):
+    n = 4096
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(2, 32, hidden)
+    order = datagen.make_order(n, 256, 2, True)
+    o1, o2 = O.train(X, Y, W1, W2, 256, LR, 2, order=order)
+    clusters = [c for c in (1, 2, 4, 8, 16) if hidden % c == 0 and hidden // c in (16, 32, 64)]
+    for cl in [0] + clusters:
+        g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 2, order=order, cluster=cl)
+        assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5, (hidden, cl, nerr(g1, o1), nerr(g2, o2))
+    lg, lo = gpu_eval(X, Y, g1, g2), O.eval_loss(X, Y, o1, o2)
+    assert abs(lg - lo) <= 1e-5 * lo
+
+
+# ------------------------------------------------------------------ config 5 shapes (batch sweep) + ragged
+@pytest.mark.parametrize("batch,n", [(32, 2048), (1024, 8192), (4096, 16384), (64, 1000), (100, 1001),
+                                     (128, 700), (300, 1000), (256, 1000), (5000, 3000), (1, 7)])
+def test_batch_sweep_and_ragged(batch, n):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(2, 32, 256)
+    order = datagen.make_order(n, batch, 2, True)
+    o1, o2 = O.train(X, Y, W1, W2, batch, LR, 2, order=order)
+    for cl in (4, 8, 16):
+        g1, g2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, cluster=cl)
+        assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5, (batch, n, cl, nerr(g1, o1), nerr(g2, o2))
+    u1, u2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=B.VARIANT_UNFUSED)
+    assert nerr(u1, o1) <= 1e-5 and nerr(u2, o2) <= 1e-5
+
+
+# ------------------------------------------------------------------ invariants on the GPU path
+def test_zero_lr_bit_identical(cfg1):
+    X, Y, W1, W2 = cfg1
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, 0.0, 3)
+    assert g1.tobytes() == W1.tobytes() and g2.tobytes() == W2.tobytes()
+
+
+def test_zero_epochs_is_noop(cfg1):
+    X, Y, W1, W2 = cfg1
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 0)
+    assert g1.tobytes() == W1.tobytes() and g2.tobytes() == W2.tobytes()
+
+
+def test_resume_and_determinism(cfg1):
+    X, Y, W1, W2 = cfg1
+    a1, a2 = gpu_train(X, Y, W1, W2, 256, LR, 2)
+    b1, b2 = gpu_train(X, Y, W1, W2, 256, LR, 1)
+    b1, b2 = gpu_train(X, Y, b1, b2, 256, LR, 1)
+    assert a1.tobytes() == b1.tobytes() and a2.tobytes() == b2.tobytes()
+    c1, c2 = gpu_train(X, Y, W1, W2, 256, LR, 2)
+    assert a1.tobytes() == c1.tobytes() and a2.tobytes() == c2.tobytes()
+
+
+def test_hand_example_embedded(golden):
+    g = golden["P1"]
+    for H in (32, 64):
+        X = np.zeros((2, 32), np.float32); X[:, :2] = g["X"]
+        W1 = np.zeros((32, H), np.float32); W1[:2, :4] = g["W1"]
+        W2 = np.zeros(H, np.float32); W2[:4] = g["W2"]
+        Y = np.array(g["Y"], np.float32)
+        w1, w2 = gpu_train(X, Y, W1, W2, 2, g["lr"], 1)
+        np.testing.assert_allclose(w1[:2, :4], np.array(g["W1_after"]), atol=3e-7)
+        np.testing.assert_allclose(w2[:4], np.array(g["W2_after"]), atol=3e-7)
+        assert not w1[2:, :].any() and not w1[:, 4:].any() and not w2[4:].any()
+        assert abs(gpu_eval(X, Y, W1, W2) - g["L"]) < 1e-5
+        assert abs(gpu_eval(X, Y, w1, w2) - g["L_after"]) < 1e-5
+
+
+def test_tie_at_zero(golden):
+    g1h, g2h = golden["P1"], golden["P2"]
+    X = np.zeros((3, 32), np.float32); X[:, :2] = g2h["X"]
+    W1 = np.zeros((32, 32), np.float32); W1[:2, :4] = g1h["W1"]
+    W2 = np.zeros(32, np.float32); W2[:4] = g1h["W2"]
+    Y = np.array(g2h["Y"], np.float32)
+    w1, w2 = gpu_train(X, Y, W1, W2, 3, 1.0, 1)           # lr = 1: W - dW
+    np.testing.assert_allclose(3 * (W1 - w1)[:2, :4], np.array(g2h["three_dW1"]), rtol=1e-6)
+    np.testing.assert_allclose(3 * (W2 - w2)[:4], np.array(g2h["three_dW2"]), rtol=1e-6)
+    assert abs(gpu_eval(X, Y, W1, W2) - g2h["L"]) < 1e-5
+
+
+# ------------------------------------------------------------------ eval pass
+@pytest.mark.parametrize("hidden", [32, 64, 128, 256, 512, 1024])
+@pytest.mark.parametrize("n", [1, 127, 5000, 70001])
+def test_eval_matches_oracle(hidden, n):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(5, 32, hidden)
+    lg, lo = gpu_eval(X, Y, W1, W2), O.eval_loss(X, Y, W1, W2)
+    assert abs(lg - lo) <= 2e-6 * lo, (hidden, n, lg, lo)
+
+
+def test_eval_closed_forms():
+    X, Y = datagen.make_dataset(50000, 0.1)
+    W1, _ = O.init_weights(5, 32, 256)
+    l0 = gpu_eval(X, Y, W1, np.zeros(256, np.float32))
+    assert abs(l0 - np.mean(Y.astype(np.float64) ** 2)) <= 1e-6 * l0        # W2 = 0 -> mean(Y^2)
+    T1, T2 = datagen.teacher()
+    lt = gpu_eval(X, Y, T1.astype(np.float32), T2.astype(np.float32).reshape(-1))
+    assert abs(lt - 0.01) < 3 * 0.01 * math.sqrt(2 / 50000) + 1e-5          # student == teacher
+
+
+def test_eval_is_deterministic():
+    X, Y = datagen.make_dataset(100000, 0.1)
+    W1, W2 = O.init_weights(5, 32, 256)
+    a = gpu_eval(X, Y, W1, W2)
+    assert all(gpu_eval(X, Y, W1, W2) == a for _ in range(3))
+
+
+# ------------------------------------------------------------------ host-buffer (end-to-end) entry points
+def test_host_entry_points(cfg1):
+    X, Y, W1, W2 = cfg1
+    B.mlp_init(2, 32, 256, 1)
+    h1, h2 = W1.copy(), W2.copy()
+    order = datagen.make_order(1024, 256, 2, True)
+    B.mlp_train_host(X, Y, 1024, 256, LR, 2, h1, h2, order.reshape(-1).copy())
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 2, order=order)
+    assert h1.tobytes() == g1.tobytes() and h2.tobytes() == g2.tobytes()
+    assert B.mlp_eval_loss_host(X, Y, 1024, h1, h2) == gpu_eval(X, Y, g1, g2)
+
+
+def test_launch_counter_counts_library_kernels(cfg1):
+    X, Y, W1, W2 = cfg1
+    before = B.mlp_launch_count()
+    gpu_train(X, Y, W1, W2, 256, LR, 1)
+    assert B.mlp_launch_count() == before + 1              # one launch for all 4 steps
+    before = B.mlp_launch_count()
+    gpu_train(X, Y, W1, W2, 256, LR, 1, variant=B.VARIANT_UNFUSED)
+    assert B.mlp_launch_count() == before + 32             # 8 kernels x 4 steps
