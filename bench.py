@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200 MLP-SGD library (contract: see DESIGN.md section 7).
+
+Workload (N=1): BASELINE.json configs[1] ("config2"): 32-256-1 ReLU/MSE MLP, fp32, batch 256,
+lr 0.002, n = 65,536 seeded teacher-student samples, 10 epochs with a per-epoch batch-order
+permutation (seed 3).  One bench "step" = one whole run of that job through the fused training
+kernel (2,560 SGD steps, one launch) followed by one eval-loss pass over the dataset.
+metric = training samples/s (whole job, all ranks).  N>1: independent replicas (the SGD step does
+not shard -- DESIGN.md section 6), weak scaling, no data-path collective.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+WORKLOAD = "config2"
+METRIC = "training samples/s (fp32, B=256, 32-256-1 MLP SGD)"
+UNIT = "samples/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_leg(cfg, X, Y, W1, W2, order, budget_s=15.0):
+    """The oracle, as it stands, on the host cores: whole epochs of the same job until ~budget_s."""
+    from oracle import mlp_oracle as O
+    t0 = time.perf_counter()
+    w1, w2 = O.train(X, Y, W1, W2, cfg.batch, cfg.lr, 1, order=order[:1])
+    t1 = time.perf_counter() - t0
+    epochs = 1
+    extra = int(min(cfg.epochs - 1, max(0, budget_s / max(t1, 1e-3) - 1)))
+    if extra > 0:
+        O.train(X, Y, w1, w2, cfg.batch, cfg.lr, extra, order=order[1:1 + extra])
+        epochs += extra
+    dt = time.perf_counter() - t0
+    return {"value": cfg.n * epochs / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{epochs} of {cfg.epochs} epochs of {cfg.name} (n={cfg.n}, {epochs * (cfg.n // cfg.batch)} SGD steps), "
+                      f"{dt:.2f} s wall", "us_per_sgd_step": dt / (epochs * (cfg.n // cfg.batch)) * 1e6}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle timed on the box's host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import mlp_oracle as O
+    from paper_2606_30497_b200 import datagen
+    cfg = datagen.CONFIGS[WORKLOAD]
+    X, Y = datagen.make_dataset(cfg.n, cfg.sigma)
+    W1, W2 = O.init_weights(2, 32, cfg.hidden)
+    order = datagen.make_order(cfg.n, cfg.batch, cfg.epochs, cfg.shuffle)
+    w1, w2 = W1, W2
+    times = []
+    for k in range(args.warmup + args.steps):
+        e = k % cfg.epochs
+        t0 = time.perf_counter()
+        w1, w2 = O.train(X, Y, w1, w2, cfg.batch, cfg.lr, 1, order=order[e:e + 1])
+        O.eval_loss(X, Y, w1, w2)
+        if k >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = sum(times)
+    value = cfg.n * args.steps / total
+    sample = (f"each step = 1 of the {cfg.epochs} epochs of {cfg.name} (65,536 samples, 256 SGD steps) "
+              f"+ one eval pass, CPU oracle fp64")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD, "n": cfg.n, "hidden": cfg.hidden, "batch": cfg.batch,
+                   "epochs_per_step": 1, "step_definition": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_30497_b200 import binding as B
+    from paper_2606_30497_b200 import datagen, roofline
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference "
+                         "for the oracle arm)")
+    torch.cuda.set_device(local_rank)
+    peaks = load_peaks()
+    cfg = datagen.CONFIGS[WORKLOAD]
+    sgd_steps = cfg.epochs * datagen.num_batches(cfg.n, cfg.batch)
+    samples_per_step = cfg.n * cfg.epochs
+
+    # ---- seeded synthetic inputs (same bytes on every rank: independent replicas) ----
+    X, Y = datagen.make_dataset(cfg.n, cfg.sigma)
+    order = datagen.make_order(cfg.n, cfg.batch, cfg.epochs, cfg.shuffle)
+    B.mlp_init(2, 32, cfg.hidden, 1)
+    dX, dY = torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()
+    dO = torch.from_numpy(order.reshape(-1).copy()).cuda()
+    W1i = torch.empty(32, cfg.hidden, device="cuda"); W2i = torch.empty(cfg.hidden, device="cuda")
+    B.mlp_init_weights(W1i, W2i)
+    d1, d2 = W1i.clone(), W2i.clone()
+    dloss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    cluster = B.mlp_get_cluster()
+
+    def one_step(ev=None):
+        d1.copy_(W1i); d2.copy_(W2i)
+        flush.zero_()                                   # evict the dataset from L2 (untimed)
+        if ev: ev[0].record()
+        B.mlp_train_ex(dX, dY, cfg.n, cfg.batch, cfg.lr, cfg.epochs, d1, d2, dO, B.VARIANT_FUSED)
+        if ev: ev[1].record()
+        B.mlp_eval_loss_async(dX, dY, cfg.n, d1, d2, dloss, B.VARIANT_FUSED)
+        if ev: ev[2].record()
+
+    for _ in range(args.warmup):
+        one_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = B.mlp_launch_count()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        one_step(evs[k])
+    torch.cuda.synchronize()
+    launches = B.mlp_launch_count() - launches0
+    sampler.stop()
+    if world > 1:
+        dist.barrier()
+    train_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    step_ms = [e[0].elapsed_time(e[2]) for e in evs]
+    total_ms = sum(step_ms)
+    stats = B.mlp_get_train_stats()
+    final_loss = float(dloss.item())
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    if rank != 0:
+        return
+
+    value = world * samples_per_step * args.steps / (total_ms * 1e-3)
+    train_ms_avg = sum(train_ms) / len(train_ms)
+    us_per_sgd = train_ms_avg * 1e3 / sgd_steps
+    kernel_mhz = stats["sm_cycles"] / stats["ns"] * 1e3 if stats["ns"] else None
+
+    # ---- roofline of the dominant kernel (fused training kernel; ALU-bound) ----
+    flop_launch = roofline.f_step(cfg.batch, cfg.hidden) * sgd_steps
+    achieved = flop_launch / (train_ms_avg * 1e-3) / 1e12
+    peak = roofline.FMA_FLOP_PER_CLK_PER_SM * cluster * peaks["sm_max_mhz"] * 1e6 / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("train_fused_dram_bytes_per_launch")
+    roof = {"bound": "alu", "kernel": "k_train_fused", "achieved": achieved, "peak": peak,
+            "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+            "peak_source": f"256 FLOP/clk/SM x {cluster} occupied SMs x sm_max_mhz "
+                           f"({peaks['sm_max_mhz']:.0f}, {peaks['source']})",
+            "us_per_sgd_step": us_per_sgd,
+            "floor_us_per_sgd_step": roofline.train_floor_us(cfg.batch, cfg.hidden, cluster, peaks["sm_max_mhz"]),
+            "cluster": cluster, "sm_mhz_in_kernel": kernel_mhz,
+            "algorithmic_hbm_bytes_per_launch": roofline.step_bytes(cfg.batch) * sgd_steps}
+
+    # ---- eval kernel on BASELINE.json configs[4]'s 4,194,304 x 32 matrix (HBM measurement) ----
+    n5 = 1 << 22
+    gen = torch.Generator(device="cuda"); gen.manual_seed(0)
+    X5 = torch.randn(n5, 32, device="cuda", generator=gen)
+    Y5 = torch.randn(n5, device="cuda", generator=gen)
+    best = {}
+    for variant, name in ((B.VARIANT_FUSED, "fp32"), (B.VARIANT_TF32, "tf32")):
+        try:
+            B.mlp_eval_loss_async(X5, Y5, n5, d1, d2, dloss, variant)
+        except B.MlpError:
+            continue
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(10):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); B.mlp_eval_loss_async(X5, Y5, n5, d1, d2, dloss, variant); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        ms = min(ts)
+        gbs = n5 * roofline.eval_bytes_per_sample() / (ms * 1e-3) / 1e9
+        tf = n5 * roofline.eval_flop_per_sample(cfg.hidden) / (ms * 1e-3) / 1e12
+        best[name] = {"us": ms * 1e3, "GB/s": gbs, "frac_of_measured_hbm": gbs / peaks["hbm_gbs"],
+                      "frac_of_8TBs_nominal": gbs / 8000.0, "TFLOP/s": tf,
+                      "frac_of_fp32_fma_peak": tf / (256 * 148 * peaks["sm_max_mhz"] * 1e6 / 1e12)}
+    del X5, Y5
+
+    # ---- end-to-end: the same job through the host-buffer C-ABI call, copies inside the timed region ----
+    hX = torch.from_numpy(X).pin_memory(); hY = torch.from_numpy(Y).pin_memory()
+    hO = torch.from_numpy(order.reshape(-1).copy()).pin_memory()
+    h1 = W1i.cpu().pin_memory(); h2 = W2i.cpu().pin_memory()
+    w1_init, w2_init = h1.clone(), h2.clone()
+    for _ in range(2):
+        h1.copy_(w1_init); h2.copy_(w2_init)
+        B.mlp_train_host(hX, hY, cfg.n, cfg.batch, cfg.lr, cfg.epochs, h1, h2, hO)
+    e2e_t = 0.0
+    for _ in range(args.steps):
+        h1.copy_(w1_init); h2.copy_(w2_init)
+        t0 = time.perf_counter()
+        B.mlp_train_host(hX, hY, cfg.n, cfg.batch, cfg.lr, cfg.epochs, h1, h2, hO)
+        e2e_t += time.perf_counter() - t0
+    wbytes = (32 * cfg.hidden + cfg.hidden) * 4
+    e2e = {"value": world * samples_per_step * args.steps / e2e_t, "unit": UNIT,
+           "h2d_bytes_per_step": cfg.n * 132 + wbytes + order.size * 4, "d2h_bytes_per_step": wbytes,
+           "api": "mlp_train_host (pinned host X/Y/W/order in, trained W out)", "timer": "host wall clock"}
+    e2e_matches = bool(torch.equal(h1.cuda(), d1) and torch.equal(h2.cuda(), d2))
+
+    # ---- our unfused baseline (row a-U), a few hundred SGD steps, for context ----
+    u1, u2 = W1i.clone(), W2i.clone()
+    B.mlp_train_ex(dX, dY, cfg.n, cfg.batch, cfg.lr, 1, u1, u2, dO, B.VARIANT_UNFUSED)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); B.mlp_train_ex(dX, dY, cfg.n, cfg.batch, cfg.lr, 1, u1, u2, dO, B.VARIANT_UNFUSED); b.record()
+    torch.cuda.synchronize()
+    unfused_us = a.elapsed_time(b) * 1e3 / datagen.num_batches(cfg.n, cfg.batch)
+
+    cpu = oracle_leg(cfg, X, Y, W1i.cpu().numpy(), W2i.cpu().numpy(), order)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "n": cfg.n, "hidden": cfg.hidden, "batch": cfg.batch,
+                   "epochs": cfg.epochs, "sgd_steps_per_step": sgd_steps,
+                   "step_definition": "one full run of BASELINE.json configs[1] (10 epochs, one fused "
+                                      "launch) + one eval-loss pass",
+                   "l2": "flushed between timed steps (256 MiB memset, untimed)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU, cluster of %d SMs" % cluster},
+        "us_per_sgd_step": us_per_sgd, "final_loss": final_loss,
+        "roofline": roof, "eval_4M_rows": best, "e2e": e2e, "e2e_bitwise_equal_to_device_path": e2e_matches,
+        "gpu_launches": int(launches), "unfused_baseline_us_per_sgd_step": unfused_us,
+        "cpu_baseline": cpu, "clocks": sampler.summary(),
+        "context": "paper (Tesla T4, optimised kernels): 1,482 us/step, 172.7 k samples/s (PAPER.md:330, derived)",
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3                                  # timing rule: W >= 3
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl")
+    try:
+        run_ours(args, rank, world, local_rank)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
