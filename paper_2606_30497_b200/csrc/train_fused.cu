@@ -3,26 +3,29 @@
 // One thread-block cluster of C CTAs (one per SM) runs EVERY SGD step of mlp_train in a single
 // launch (PAPER.md:108-112 loop; eqs. 1-9).  The hidden dimension is split over
 // the cluster: CTA c owns S = hidden/C hidden units, i.e. W1[:, cS:(c+1)S] and W2[cS:(c+1)S],
-// which stay on chip (registers + shared memory) for the whole run.
+// whose fp32 master copy stays in shared memory for the whole run.
 //
-// Mapping inside a CTA (8 warps):
-//   * a lane owns TWO hidden units (u0 = lu, u1 = lu + LPS, lu = lane % LPS, LPS = S/2) and keeps
-//     their W1 columns (2 x 32 floats) and dW1 accumulators (2 x 32 floats) in registers, as
-//     16 + 16 packed fp32x2 pairs over consecutive inputs (i, i+1), so eq. 1 and eq. 8 run on
-//     FFMA2 (fma.rn.f32x2): one issue slot per two FMAs;
-//   * a warp owns BT/8 rows of the batch tile and walks them SPW = 32/LPS rows at a time; the X
-//     row is read from shared memory with broadcast 128-bit loads;
-//   * H = ReLU(Z1) for the warp's rows stays in registers between forward and backward.
+// Mapping inside a CTA (8 warps), v2:
+//   * a lane owns FOUR hidden units (u_j = lu + j*LPS, lu = lane % LPS, LPS = S/4).  During the
+//     forward pass it holds their W1 columns (4 x 32 floats) in registers, during the backward
+//     pass the same registers hold the dW1 accumulators: the two live ranges never overlap, so a
+//     128-bit shared-memory load of X feeds 8 FFMA2 (fma.rn.f32x2) instead of v1's 4 -- on
+//     sm_100a an LDS.128 costs 2 cycles of the SM's shared-memory pipe, 8 FFMA2 cost 4 cycles of
+//     the FMA pipes, so the FMA pipe is the binding unit (profiles/r01_ncu_v1.md);
+//   * a warp instruction covers SPW = 32/LPS rows (one per lane sub-group s = lane / LPS).  The
+//     X tile is stored as SPW blocks of BT/SPW rows, block s shifted by 16*s bytes, so the SPW
+//     rows read by one LDS.128 fall into distinct bank groups (no conflict, no swizzle);
+//   * H = ReLU(Z1) of the warp's rows stays in registers between forward and backward.
 // Per tile: forward (eqs. 1-3) -> per-row partial Ypred reduced across the LPS lanes with a
 // transposing shuffle tree -> pushed to every CTA of the cluster with st.async (DSMEM store that
 // completes transaction bytes on the destination's mbarrier: one hop, no flag) -> every CTA sums
 // the C partials in rank order -> dZ2 (eq. 5) -> dW2, dZ1, dW1 (eqs. 6-8) accumulated in
 // registers.  The tile is processed as NSPLIT row groups so that the exchange of one group is in
-// flight while the other group computes.  At the end of the batch the 8 warps' partial gradients
-// are summed through shared memory in a fixed order (deterministic), eq. 9 is applied to the
-// shared-memory master copy and the warps re-load their columns.
-// X tiles arrive by cp.async.bulk (TMA engine) into a 2-deep ring, one tile ahead; batches with
-// more than BT rows are processed as several tiles with the gradients kept in registers.
+// flight while the other group computes.  After the backward pass the SPW sub-groups' partial
+// dW1 are combined with a transposing butterfly (each lane ends with 1/SPW of the sums), added
+// to the warp's shared-memory partial; at the end of the batch the 8 warps' partials are summed
+// in a fixed order (deterministic), eq. 9 is applied to the shared-memory master copy.
+// X tiles arrive by cp.async.bulk (TMA engine) into a 2-deep ring, one tile ahead.
 #include "common.cuh"
 #include "internal.h"
 
@@ -69,19 +72,37 @@ struct GroupReduce {
     }
 };
 
-__device__ __forceinline__ f32x2 shfl_xor2(f32x2 v, int o) {
-    return __shfl_xor_sync(0xffffffffu, v, o);
-}
+// Transposing butterfly over the SPW row sub-groups of a warp (lane = s*LPS + lu): NV packed
+// pairs per lane in, NV/SPW out; the lane of sub-group s ends with the totals of the original
+// entries SPW*k + s, k = 0..NV/SPW-1.
+template <int NV, int SPW, int LPS, int R = 1>
+struct SubgroupReduce {
+    static __device__ __forceinline__ void run(f32x2* v, int s) {
+        if constexpr (R < SPW) {
+            const bool up = (s & R) != 0;
+#pragma unroll
+            for (int k = 0; k < NV / 2; ++k) {
+                const f32x2 keep = up ? v[2 * k + 1] : v[2 * k];
+                const f32x2 send = up ? v[2 * k] : v[2 * k + 1];
+                v[k] = fadd2(keep, __shfl_xor_sync(0xffffffffu, send, LPS * R));
+            }
+            SubgroupReduce<NV / 2, SPW, LPS, R * 2>::run(v, s);
+        }
+    }
+};
 
 template <int S, int BT, int NSPLIT>
 __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p) {
-    constexpr int LPS = S / 2;            // lanes per sample row
-    constexpr int SPW = 32 / LPS;         // sample rows per warp instruction
-    constexpr int RPW = BT / kWarps;      // rows per warp per tile
-    constexpr int ITER = RPW / SPW;       // row groups per warp per tile
-    constexpr int ITS = ITER / NSPLIT;    // row groups per exchange sub-tile
-    static_assert(LPS >= 8 && LPS <= 32 && RPW % SPW == 0 && ITER % NSPLIT == 0 && ITS >= 1, "cfg");
-    static_assert(ITS <= LPS, "transposing reduction needs ITS <= LPS");
+    constexpr int LPS = S / 4;            // lanes per sample row
+    constexpr int SPW = 32 / LPS;         // sample rows per warp instruction (row sub-groups)
+    constexpr int RB = BT / SPW;          // rows per X block (one block per sub-group)
+    constexpr int ITER = RB / kWarps;     // rows per lane per tile
+    constexpr int ITS = ITER / NSPLIT;    // rows per lane per exchange sub-tile
+    constexpr int XBLK = RB * kIn + 4;    // floats per X block incl. the 16-byte stagger
+    constexpr int XSTAGE = SPW * XBLK;    // floats per ring stage
+    constexpr int CPL = 8 / SPW;          // 4-input chunks of dW1 per unit a lane ends up with
+    static_assert(LPS >= 4 && LPS <= 32 && RB % kWarps == 0 && ITER >= 1 && ITER % NSPLIT == 0, "cfg");
+    static_assert(ITS >= 1 && ITS <= LPS, "transposing reduction needs ITS <= LPS");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -89,8 +110,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     const uint32_t crank = cluster_ctarank(), C = cluster_nctarank();
     const int H = p.H;
 
-    float* Xs = reinterpret_cast<float*>(smem_raw);          // [2][BT*32]
-    float* ypp = Xs + 2 * BT * kIn;                           // [2][C][BT]
+    float* Xs = reinterpret_cast<float*>(smem_raw);          // [2][XSTAGE]
+    float* ypp = Xs + 2 * XSTAGE;                             // [2][C][BT]
     float* part = ypp + 2 * C * BT;                           // [kWarps][S*32]  layout [q][u][4]
     float* part2 = part + kWarps * S * kIn;                   // [kWarps][S]
     float* W1s = part2 + kWarps * S;                          // [S*32]          layout [q][u][4]
@@ -103,7 +124,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     if (crank == 0 && tid == 0) { clk0 = clock64(); ns0 = globaltimer_ns(); }
 
     // ---- one-time setup: zero the X ring, load this CTA's weight slice, init barriers ----------
-    for (int f = tid; f < 2 * BT * kIn; f += kThreads) Xs[f] = 0.f;
+    for (int f = tid; f < 2 * XSTAGE; f += kThreads) Xs[f] = 0.f;
     for (int f = tid; f < S * kIn; f += kThreads) {
         const int q = f / (S * 4), rem = f % (S * 4), u = rem >> 2, i = q * 4 + (rem & 3);
         W1s[f] = p.W1[(size_t)i * H + crank * S + u];
@@ -122,38 +143,32 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     __syncthreads();
     cluster_sync_all();        // every CTA's barriers exist before anyone pushes to them
 
-    // ---- per-lane weight registers ---------------------------------------------------------------
-    f32x2 w0[16], w1[16];      // W1 columns of u0, u1 as (i, i+1) pairs
-    float w2r0, w2r1;
-    auto reload_weights = [&]() {
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(W1s + (q * S + lu) * 4);
-            const ulonglong2 b = *reinterpret_cast<const ulonglong2*>(W1s + (q * S + lu + LPS) * 4);
-            w0[2 * q] = a.x; w0[2 * q + 1] = a.y;
-            w1[2 * q] = b.x; w1[2 * q + 1] = b.y;
-        }
-        w2r0 = W2s[lu];
-        w2r1 = W2s[lu + LPS];
-    };
-    reload_weights();
-
     const long long total = p.total_steps;
     auto batch_index = [&](long long step) -> int {
         return p.order ? __ldg(p.order + step) : (int)(step % p.nb);
     };
+    // producer (one thread): bring `rows` rows starting at global row g0 into ring stage nbuf
+    auto issue_tile = [&](long long g0, int rows, unsigned nbuf) {
+        const uint32_t bar = bar_full + 8 * nbuf;
+        mbar_arrive_expect_tx(bar, rows * 128);
+#pragma unroll
+        for (int b = 0; b < SPW; ++b) {
+            const int rb = min(RB, rows - b * RB);
+            if (rb > 0)
+                bulk_g2s(smem_u32(Xs + nbuf * XSTAGE + b * XBLK), p.X + (g0 + b * RB) * kIn,
+                         rb * 128, bar);
+        }
+    };
     int t_cur = batch_index(0);
     int t_next = total > 1 ? batch_index(1) : 0;
-
-    // producer state: issue tile 0
     if (warp == 0 && lane == 0) {
         const long long r0 = (long long)t_cur * p.B;
         const int m = (int)min((long long)p.B, p.n - r0);
-        const int rows = min(BT, m);
-        mbar_arrive_expect_tx(bar_full, rows * 128);
-        bulk_g2s(smem_u32(Xs), p.X + r0 * kIn, rows * 128, bar_full);
+        issue_tile(r0, min(BT, m), 0);
     }
 
+    const int rowl = warp * ITER;                     // first row of this lane inside its block
+    float* mypart = part + warp * (S * kIn);
     unsigned gt = 0;   // global tile counter
     for (long long step = 0; step < total; ++step) {
         const int t_nn = (step + 2 < total) ? batch_index(step + 2) : 0;
@@ -161,17 +176,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
         const int m = (int)min((long long)p.B, p.n - r0);
         const int ntiles = (m + BT - 1) / BT;
         const float scale = 2.0f / (float)m;                  // eq. 5
-
-        f32x2 acc0[16], acc1[16];                             // dW1 partials of u0, u1 (eq. 8)
-#pragma unroll
-        for (int k = 0; k < 16; ++k) { acc0[k] = 0ull; acc1[k] = 0ull; }
-        float g20 = 0.f, g21 = 0.f;                           // dW2 partials (eq. 6)
+        float g2[4] = {0.f, 0.f, 0.f, 0.f};                   // dW2 partials (eq. 6)
 
         for (int j = 0; j < ntiles; ++j, ++gt) {
             const unsigned buf = gt & 1u, ph = (gt >> 1) & 1u;
             const int vt = min(BT, m - j * BT);               // valid rows in this tile
-            const float* Xt = Xs + buf * (BT * kIn);
+            const float* Xl = Xs + buf * XSTAGE + s * XBLK + rowl * kIn;   // this lane's rows
             const float* ypt = ypp + buf * (C * BT);
+            const int row0 = s * RB + rowl;                   // tile row of this lane's first row
 
             if (warp == 0 && lane == 0) {
                 // arm this tile's exchange barriers
@@ -188,9 +200,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                 if (have) {
                     const unsigned g1 = gt + 1, nbuf = g1 & 1u;
                     if (g1 >= 2) mbar_wait(bar_empty + 8 * nbuf, ((g1 >> 1) - 1) & 1u);
-                    mbar_arrive_expect_tx(bar_full + 8 * nbuf, nrows * 128);
-                    bulk_g2s(smem_u32(Xs + nbuf * (BT * kIn)), p.X + nr0 * kIn, nrows * 128,
-                             bar_full + 8 * nbuf);
+                    issue_tile(nr0, nrows, nbuf);
                 }
             }
             __syncwarp();
@@ -199,54 +209,80 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             float yv[NSPLIT];
 #pragma unroll
             for (int q = 0; q < NSPLIT; ++q) {
-                const int row = warp * RPW + (q * ITS + (lu & (ITS - 1))) * SPW + s;
+                const int row = row0 + q * ITS + (lu & (ITS - 1));
                 yv[q] = row < vt ? __ldg(p.Y + r0 + (long long)j * BT + row) : 0.f;
             }
 
-            mbar_wait(bar_full + 8 * buf, ph);
-
-            // ---------------- forward: eqs. 1-3 ----------------
-            float hreg[ITER][2];
+            float hreg[ITER][4];
+            float w2r[4];
 #pragma unroll
-            for (int q = 0; q < NSPLIT; ++q) {
-                float pv[ITS];
+            for (int u = 0; u < 4; ++u) w2r[u] = W2s[lu + u * LPS];
+            {
+                // ---------------- forward: eqs. 1-3 (W1 columns in registers) ----------------
+                f32x2 w[4][16];
 #pragma unroll
-                for (int k = 0; k < ITS; ++k) {
-                    const int it = q * ITS + k;
-                    const int row = warp * RPW + it * SPW + s;
-                    const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xt + row * kIn);
-                    f32x2 a0 = 0ull, a1 = 0ull;
+                for (int q = 0; q < 8; ++q)
 #pragma unroll
-                    for (int x = 0; x < 8; ++x) {
-                        const ulonglong2 xv = xrow[x];
-                        ffma2(a0, xv.x, w0[2 * x]); ffma2(a1, xv.x, w1[2 * x]);
-                        ffma2(a0, xv.y, w0[2 * x + 1]); ffma2(a1, xv.y, w1[2 * x + 1]);
+                    for (int u = 0; u < 4; ++u) {
+                        const ulonglong2 a =
+                            *reinterpret_cast<const ulonglong2*>(W1s + (q * S + lu + u * LPS) * 4);
+                        w[u][2 * q] = a.x; w[u][2 * q + 1] = a.y;
                     }
-                    const bool valid = row < vt;
-                    const float h0 = valid ? fmaxf(hsum2(a0), 0.f) : 0.f;     // eq. 2
-                    const float h1 = valid ? fmaxf(hsum2(a1), 0.f) : 0.f;
-                    hreg[it][0] = h0; hreg[it][1] = h1;
-                    pv[k] = fmaf(h1, w2r1, h0 * w2r0);                        // eq. 3 (partial)
-                }
-                GroupReduce<ITS, LPS>::run(pv, lu);
-                if (lu < ITS) {
-                    const int row = warp * RPW + (q * ITS + lu) * SPW + s;
-                    const uint32_t dst = smem_u32(ypp + buf * (C * BT) + crank * BT + row);
-                    const uint32_t bar = bar_yp + 8 * (buf * NSPLIT + q);
-                    for (uint32_t dd = 0; dd < C; ++dd) {
-                        const uint32_t d = (crank + dd) % C;
-                        st_async_f32(mapa(dst, d), pv[0], mapa(bar, d));
+                mbar_wait(bar_full + 8 * buf, ph);
+#pragma unroll
+                for (int q = 0; q < NSPLIT; ++q) {
+                    float pv[ITS];
+#pragma unroll
+                    for (int k = 0; k < ITS; ++k) {
+                        const int it = q * ITS + k;
+                        const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xl + it * kIn);
+                        f32x2 a[4] = {0ull, 0ull, 0ull, 0ull};
+#pragma unroll
+                        for (int x = 0; x < 8; ++x) {
+                            const ulonglong2 xv = xrow[x];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (x == 0) a[u] = fmul2(xv.x, w[u][0]);                // eq. 1
+                                else ffma2(a[u], xv.x, w[u][2 * x]);
+                                ffma2(a[u], xv.y, w[u][2 * x + 1]);
+                            }
+                        }
+                        float pr = 0.f;
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const float h = fmaxf(hsum2(a[u]), 0.f);                     // eq. 2
+                            hreg[it][u] = h;
+                            pr = fmaf(h, w2r[u], pr);                                    // eq. 3
+                        }
+                        pv[k] = pr;
+                    }
+                    GroupReduce<ITS, LPS>::run(pv, lu);
+                    if (lu < ITS) {
+                        const int row = row0 + q * ITS + lu;
+                        const uint32_t dst = smem_u32(ypp + buf * (C * BT) + crank * BT + row);
+                        const uint32_t bar = bar_yp + 8 * (buf * NSPLIT + q);
+                        for (uint32_t dd = 0; dd < C; ++dd) {
+                            const uint32_t d = (crank + dd) % C;
+                            st_async_f32(mapa(dst, d), pv[0], mapa(bar, d));
+                        }
                     }
                 }
             }
 
-            // ---------------- backward: eqs. 5-8 ----------------
+            // ---------------- backward: eqs. 5-8 (the same registers now hold dW1) ----------------
+            // acc[AI(u, kk)] accumulates dW1 for unit u and the input pair (2kk, 2kk+1); the flat
+            // order is the one SubgroupReduce transposes (see AI below).
+            f32x2 acc[64];
+            auto AI = [](int u, int kk) constexpr -> int {
+                const int q = kk >> 1, hb = kk & 1, c2 = q / SPW, sp = q % SPW;
+                return SPW * ((u * CPL + c2) * 2 + hb) + sp;
+            };
 #pragma unroll
             for (int q = 0; q < NSPLIT; ++q) {
                 mbar_wait_cluster(bar_yp + 8 * (buf * NSPLIT + q), ph);
                 float dzv;
                 {
-                    const int row = warp * RPW + (q * ITS + (lu & (ITS - 1))) * SPW + s;
+                    const int row = row0 + q * ITS + (lu & (ITS - 1));
                     float yp = 0.f;
                     for (uint32_t c = 0; c < C; ++c) yp += ypt[c * BT + row];  // fixed rank order
                     dzv = row < vt ? scale * (yp - yv[q]) : 0.f;              // eq. 5
@@ -254,52 +290,61 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 #pragma unroll
                 for (int k = 0; k < ITS; ++k) {
                     const int it = q * ITS + k;
-                    const int row = warp * RPW + it * SPW + s;
                     const float d = __shfl_sync(0xffffffffu, dzv, (lane & ~(LPS - 1)) | k);
-                    const float h0 = hreg[it][0], h1 = hreg[it][1];
-                    g20 = fmaf(h0, d, g20);                                    // eq. 6
-                    g21 = fmaf(h1, d, g21);
-                    const float e0 = h0 > 0.f ? d * w2r0 : 0.f;                // eq. 7 (old W2)
-                    const float e1 = h1 > 0.f ? d * w2r1 : 0.f;
-                    const f32x2 dd0 = pack2(e0, e0), dd1 = pack2(e1, e1);
-                    const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xt + row * kIn);
+                    f32x2 dd[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const float h = hreg[it][u];
+                        g2[u] = fmaf(h, d, g2[u]);                             // eq. 6
+                        const float e = h > 0.f ? d * w2r[u] : 0.f;            // eq. 7 (old W2)
+                        dd[u] = pack2(e, e);
+                    }
+                    const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xl + it * kIn);
 #pragma unroll
                     for (int x = 0; x < 8; ++x) {                              // eq. 8
                         const ulonglong2 xv = xrow[x];
-                        ffma2(acc0[2 * x], xv.x, dd0); ffma2(acc1[2 * x], xv.x, dd1);
-                        ffma2(acc0[2 * x + 1], xv.y, dd0); ffma2(acc1[2 * x + 1], xv.y, dd1);
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (it == 0) {
+                                acc[AI(u, 2 * x)] = fmul2(xv.x, dd[u]);
+                                acc[AI(u, 2 * x + 1)] = fmul2(xv.y, dd[u]);
+                            } else {
+                                ffma2(acc[AI(u, 2 * x)], xv.x, dd[u]);
+                                ffma2(acc[AI(u, 2 * x + 1)], xv.y, dd[u]);
+                            }
+                        }
                     }
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + 8 * buf);   // this warp is done with the X tile
+
+            // combine the SPW sub-groups; lane (s, lu) ends with chunks q = SPW*c2 + s of its units
+            SubgroupReduce<64, SPW, LPS>::run(acc, s);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int c2 = 0; c2 < CPL; ++c2) {
+                    const int q = SPW * c2 + s;
+                    ulonglong2* dst = reinterpret_cast<ulonglong2*>(mypart + (q * S + lu + u * LPS) * 4);
+                    f32x2 lo = acc[(u * CPL + c2) * 2], hi = acc[(u * CPL + c2) * 2 + 1];
+                    if (j > 0) {                               // later tiles of a large batch
+                        const ulonglong2 old = *dst;
+                        lo = fadd2(lo, old.x); hi = fadd2(hi, old.y);
+                    }
+                    *dst = make_ulonglong2(lo, hi);
+                }
         }
 
         // ---------------- end of batch: reduce partial gradients, eq. 9 ----------------
-        if constexpr (SPW > 1) {
-            const f32x2 one = pack2(1.f, 1.f);
 #pragma unroll
-            for (int o = LPS; o < 32; o <<= 1) {
+        for (int o = LPS; o < 32; o <<= 1)
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    ffma2(acc0[k], shfl_xor2(acc0[k], o), one);
-                    ffma2(acc1[k], shfl_xor2(acc1[k], o), one);
-                }
-                g20 += __shfl_xor_sync(0xffffffffu, g20, o);
-                g21 += __shfl_xor_sync(0xffffffffu, g21, o);
-            }
+            for (int u = 0; u < 4; ++u) g2[u] += __shfl_xor_sync(0xffffffffu, g2[u], o);
+        if (s == 0) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) part2[warp * S + lu + u * LPS] = g2[u];
         }
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            // after the reduction every sub-sample group holds the sums: spread the stores
-            if (s == (q * SPW) / 16)
-                *reinterpret_cast<ulonglong2*>(part + ((warp * 8 + q) * S + lu) * 4) =
-                    make_ulonglong2(acc0[2 * q], acc0[2 * q + 1]);
-            if (s == ((8 + q) * SPW) / 16)
-                *reinterpret_cast<ulonglong2*>(part + ((warp * 8 + q) * S + lu + LPS) * 4) =
-                    make_ulonglong2(acc1[2 * q], acc1[2 * q + 1]);
-        }
-        if (s == 0) { part2[warp * S + lu] = g20; part2[warp * S + lu + LPS] = g21; }
         __syncthreads();
         for (int f = tid; f < S * 8; f += kThreads) {
             float4 sum = reinterpret_cast<const float4*>(part)[f];
@@ -319,7 +364,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             W2s[tid] -= p.lr * sum;                                            // eq. 9
         }
         __syncthreads();
-        reload_weights();
         t_cur = t_next;
         t_next = t_nn;
     }
@@ -339,11 +383,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     cluster_sync_all();        // no CTA exits while peers may still push into its shared memory
 }
 
-template <int S, int BT, int NSPLIT>
+template <int S, int BT>
 cudaError_t launch_cfg(const TrainParams& p, int cluster, cudaStream_t stream) {
+    constexpr int SPW = 32 / (S / 4);
+    constexpr int ITER = BT / SPW / kWarps;
+    constexpr int NSPLIT = ITER >= 2 ? 2 : 1;
     auto kern = k_train_fused<S, BT, NSPLIT>;
-    const size_t smem = sizeof(float) * (2 * BT * kIn + 2 * cluster * BT + kWarps * S * kIn +
-                                         kWarps * S + S * kIn + S) + 8 * (4 + 2 * NSPLIT);
+    const size_t smem = sizeof(float) * (2 * (BT * kIn + SPW * 4) + 2 * cluster * BT +
+                                         kWarps * S * kIn + kWarps * S + S * kIn + S) +
+                        8 * (4 + 2 * NSPLIT);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     if (cluster > 8) {
@@ -365,13 +413,28 @@ cudaError_t launch_cfg(const TrainParams& p, int cluster, cudaStream_t stream) {
     return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
+// Tile height: the smallest power of two >= batch inside [8*SPW, 64*SPW] (at most 256); 64*SPW
+// rows keep H = ReLU(Z1) of a tile in 32 registers per lane.
 template <int S>
 cudaError_t launch_s(const TrainParams& p, int cluster, cudaStream_t stream) {
     const int B = p.B;
-    if (B > 128) return launch_cfg<S, 256, 2>(p, cluster, stream);
-    if (B > 64) return launch_cfg<S, 128, 2>(p, cluster, stream);
-    if (B > 32) return launch_cfg<S, 64, (64 / kWarps) / (64 / S) >= 4 ? 2 : 1>(p, cluster, stream);
-    return launch_cfg<S, 32, 1>(p, cluster, stream);
+    if constexpr (S == 16) {
+        if (B > 128) return launch_cfg<16, 256>(p, cluster, stream);
+        if (B > 64) return launch_cfg<16, 128>(p, cluster, stream);
+        return launch_cfg<16, 64>(p, cluster, stream);
+    } else if constexpr (S == 32) {
+        if (B > 128) return launch_cfg<32, 256>(p, cluster, stream);
+        if (B > 64) return launch_cfg<32, 128>(p, cluster, stream);
+        if (B > 32) return launch_cfg<32, 64>(p, cluster, stream);
+        return launch_cfg<32, 32>(p, cluster, stream);
+    } else if constexpr (S == 64) {
+        if (B > 64) return launch_cfg<64, 128>(p, cluster, stream);
+        if (B > 32) return launch_cfg<64, 64>(p, cluster, stream);
+        return launch_cfg<64, 32>(p, cluster, stream);
+    } else {
+        if (B > 32) return launch_cfg<128, 64>(p, cluster, stream);
+        return launch_cfg<128, 32>(p, cluster, stream);
+    }
 }
 
 }  // namespace
@@ -380,7 +443,7 @@ bool fused_supported(int hidden, int cluster) {
     if (cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8 && cluster != 16) return false;
     if (hidden % cluster) return false;
     const int S = hidden / cluster;
-    return S == 16 || S == 32 || S == 64;
+    return S == 16 || S == 32 || S == 64 || S == 128;
 }
 
 int fused_default_cluster(int hidden) {
@@ -410,6 +473,7 @@ cudaError_t launch_train_fused(const float* X, const float* Y, int64_t n, int ba
         case 16: err = launch_s<16>(p, cluster, stream); break;
         case 32: err = launch_s<32>(p, cluster, stream); break;
         case 64: err = launch_s<64>(p, cluster, stream); break;
+        case 128: err = launch_s<128>(p, cluster, stream); break;
         default: return cudaErrorInvalidValue;
     }
     if (err == cudaSuccess) ++*launches;

@@ -125,7 +125,7 @@ def test_hidden_sweep(hidden):
     W1, W2 = O.init_weights(2, 32, hidden)
     order = datagen.make_order(n, 256, 2, True)
     o1, o2 = O.train(X, Y, W1, W2, 256, LR, 2, order=order)
-    clusters = [c for c in (1, 2, 4, 8, 16) if hidden % c == 0 and hidden // c in (16, 32, 64)]
+    clusters = [c for c in (1, 2, 4, 8, 16) if hidden % c == 0 and hidden // c in (16, 32, 64, 128)]
     for cl in [0] + clusters:
         g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 2, order=order, cluster=cl)
         assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5, (hidden, cl, nerr(g1, o1), nerr(g2, o2))
@@ -141,7 +141,7 @@ def test_batch_sweep_and_ragged(batch, n):
     W1, W2 = O.init_weights(2, 32, 256)
     order = datagen.make_order(n, batch, 2, True)
     o1, o2 = O.train(X, Y, W1, W2, batch, LR, 2, order=order)
-    for cl in (4, 8, 16):
+    for cl in (2, 4, 8, 16):
         g1, g2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, cluster=cl)
         assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5, (batch, n, cl, nerr(g1, o1), nerr(g2, o2))
     u1, u2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=B.VARIANT_UNFUSED)
