@@ -25,7 +25,7 @@
 // dW1 are combined with a transposing butterfly (each lane ends with 1/SPW of the sums), added
 // to the warp's shared-memory partial; at the end of the batch the 8 warps' partials are summed
 // in a fixed order (deterministic), eq. 9 is applied to the shared-memory master copy.
-// X tiles arrive by cp.async.bulk (TMA engine) into a 2-deep ring, one tile ahead.
+// X tiles arrive by cp.async.bulk (TMA engine) into a 3-stage ring, one tile ahead.
 #include "common.cuh"
 #include "internal.h"
 
@@ -34,6 +34,7 @@ namespace {
 
 constexpr int kWarps = 8;
 constexpr int kThreads = kWarps * 32;
+constexpr int kRing = 3;      // X ring stages (prefetch distance 1, slack 1)
 
 struct TrainParams {
     const float* X;
@@ -72,25 +73,6 @@ struct GroupReduce {
     }
 };
 
-// Transposing butterfly over the SPW row sub-groups of a warp (lane = s*LPS + lu): NV packed
-// pairs per lane in, NV/SPW out; the lane of sub-group s ends with the totals of the original
-// entries SPW*k + s, k = 0..NV/SPW-1.
-template <int NV, int SPW, int LPS, int R = 1>
-struct SubgroupReduce {
-    static __device__ __forceinline__ void run(f32x2* v, int s) {
-        if constexpr (R < SPW) {
-            const bool up = (s & R) != 0;
-#pragma unroll
-            for (int k = 0; k < NV / 2; ++k) {
-                const f32x2 keep = up ? v[2 * k + 1] : v[2 * k];
-                const f32x2 send = up ? v[2 * k] : v[2 * k + 1];
-                v[k] = fadd2(keep, __shfl_xor_sync(0xffffffffu, send, LPS * R));
-            }
-            SubgroupReduce<NV / 2, SPW, LPS, R * 2>::run(v, s);
-        }
-    }
-};
-
 template <int S, int BT, int NSPLIT>
 __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p) {
     constexpr int LPS = S / 4;            // lanes per sample row
@@ -100,7 +82,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     constexpr int ITS = ITER / NSPLIT;    // rows per lane per exchange sub-tile
     constexpr int XBLK = RB * kIn + 4;    // floats per X block incl. the 16-byte stagger
     constexpr int XSTAGE = SPW * XBLK;    // floats per ring stage
-    constexpr int CPL = 8 / SPW;          // 4-input chunks of dW1 per unit a lane ends up with
     static_assert(LPS >= 4 && LPS <= 32 && RB % kWarps == 0 && ITER >= 1 && ITER % NSPLIT == 0, "cfg");
     static_assert(ITS >= 1 && ITS <= LPS, "transposing reduction needs ITS <= LPS");
 
@@ -110,32 +91,32 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     const uint32_t crank = cluster_ctarank(), C = cluster_nctarank();
     const int H = p.H;
 
-    float* Xs = reinterpret_cast<float*>(smem_raw);          // [2][XSTAGE]
-    float* ypp = Xs + 2 * XSTAGE;                             // [2][C][BT]
+    float* Xs = reinterpret_cast<float*>(smem_raw);          // [kRing][XSTAGE]
+    float* ypp = Xs + kRing * XSTAGE;                         // [2][C][BT]
     float* part = ypp + 2 * C * BT;                           // [kWarps][S*32]  layout [q][u][4]
     float* part2 = part + kWarps * S * kIn;                   // [kWarps][S]
     float* W1s = part2 + kWarps * S;                          // [S*32]          layout [q][u][4]
     float* W2s = W1s + S * kIn;                               // [S]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + S);    // full[2], empty[2], yp[2][NSPLIT]
-    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + 2),
-                   bar_yp = smem_u32(bars + 4);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + S);    // full[kRing], empty[kRing], yp[2][NSPLIT]
+    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kRing),
+                   bar_yp = smem_u32(bars + 2 * kRing);
 
     unsigned long long clk0 = 0, ns0 = 0;
     if (crank == 0 && tid == 0) { clk0 = clock64(); ns0 = globaltimer_ns(); }
 
     // ---- one-time setup: zero the X ring, load this CTA's weight slice, init barriers ----------
-    for (int f = tid; f < 2 * XSTAGE; f += kThreads) Xs[f] = 0.f;
+    for (int f = tid; f < kRing * XSTAGE; f += kThreads) Xs[f] = 0.f;
     for (int f = tid; f < S * kIn; f += kThreads) {
         const int q = f / (S * 4), rem = f % (S * 4), u = rem >> 2, i = q * 4 + (rem & 3);
         W1s[f] = p.W1[(size_t)i * H + crank * S + u];
     }
     if (tid < S) W2s[tid] = p.W2[crank * S + tid];
     if (tid == 0) {
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < kRing; ++b) {
             mbar_init(bar_full + 8 * b, 1);
             mbar_init(bar_empty + 8 * b, kWarps);
-            for (int q = 0; q < NSPLIT; ++q) mbar_init(bar_yp + 8 * (b * NSPLIT + q), 1);
         }
+        for (int b = 0; b < 2 * NSPLIT; ++b) mbar_init(bar_yp + 8 * b, 1);
         fence_mbar_init();
     }
     // generic-proxy zero fill of Xs must be ordered before the async-proxy bulk copies
@@ -169,6 +150,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 
     const int rowl = warp * ITER;                     // first row of this lane inside its block
     float* mypart = part + warp * (S * kIn);
+    // Targets: lane l < ITER*SPW of a warp holds Y of the warp's row (l / ITER, l % ITER); it is
+    // fetched one tile ahead (global-load latency hidden by a whole tile) and handed to the lane
+    // that computes dZ2 by a shuffle.
+    const bool yholder = lane < ITER * SPW;
+    const int yrow = (lane / ITER) * RB + rowl + (lane % ITER);
+    float ycur = 0.f;
+    {
+        const long long r0 = (long long)t_cur * p.B;
+        const int m = (int)min((long long)p.B, p.n - r0);
+        if (yholder && yrow < min(BT, m)) ycur = __ldg(p.Y + r0 + yrow);
+    }
     unsigned gt = 0;   // global tile counter
     for (long long step = 0; step < total; ++step) {
         const int t_nn = (step + 2 < total) ? batch_index(step + 2) : 0;
@@ -179,39 +171,36 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
         float g2[4] = {0.f, 0.f, 0.f, 0.f};                   // dW2 partials (eq. 6)
 
         for (int j = 0; j < ntiles; ++j, ++gt) {
-            const unsigned buf = gt & 1u, ph = (gt >> 1) & 1u;
+            const unsigned buf = gt & 1u, ph = (gt >> 1) & 1u;       // Ypred exchange buffers
+            const unsigned xst = gt % kRing, xph = (gt / kRing) & 1u;   // X ring stage
             const int vt = min(BT, m - j * BT);               // valid rows in this tile
-            const float* Xl = Xs + buf * XSTAGE + s * XBLK + rowl * kIn;   // this lane's rows
+            const float* Xl = Xs + xst * XSTAGE + s * XBLK + rowl * kIn;   // this lane's rows
             const float* ypt = ypp + buf * (C * BT);
             const int row0 = s * RB + rowl;                   // tile row of this lane's first row
 
+            // next tile (uniform): the rest of this batch, else the first tile of the next batch
+            long long nr0 = 0; int nrows = 0;
+            if (j + 1 < ntiles) { nr0 = r0 + (long long)(j + 1) * BT; nrows = min(BT, m - (j + 1) * BT); }
+            else if (step + 1 < total) {
+                nr0 = (long long)t_next * p.B;
+                nrows = (int)min((long long)min(BT, p.B), p.n - nr0);
+            }
             if (warp == 0 && lane == 0) {
                 // arm this tile's exchange barriers
 #pragma unroll
                 for (int q = 0; q < NSPLIT; ++q)
                     mbar_arrive_expect_tx(bar_yp + 8 * (buf * NSPLIT + q), C * (BT / NSPLIT) * 4);
-                // prefetch the next tile into the other buffer
-                long long nr0; int nrows; bool have = true;
-                if (j + 1 < ntiles) { nr0 = r0 + (long long)(j + 1) * BT; nrows = min(BT, m - (j + 1) * BT); }
-                else if (step + 1 < total) {
-                    nr0 = (long long)t_next * p.B;
-                    nrows = (int)min((long long)min(BT, p.B), p.n - nr0);
-                } else { have = false; nr0 = 0; nrows = 0; }
-                if (have) {
-                    const unsigned g1 = gt + 1, nbuf = g1 & 1u;
-                    if (g1 >= 2) mbar_wait(bar_empty + 8 * nbuf, ((g1 >> 1) - 1) & 1u);
+                if (nrows > 0) {                               // prefetch X into the other buffer
+                    // stage of tile gt+1 was last read by tile gt-2: released long ago, so
+                    // this wait never holds warp 0 back behind the other warps
+                    const unsigned g1 = gt + 1, nbuf = g1 % kRing;
+                    if (g1 >= kRing) mbar_wait(bar_empty + 8 * nbuf, ((g1 / kRing) - 1) & 1u);
                     issue_tile(nr0, nrows, nbuf);
                 }
             }
             __syncwarp();
-
-            // targets of the rows whose dZ2 this lane will compute (latency hidden by the forward)
-            float yv[NSPLIT];
-#pragma unroll
-            for (int q = 0; q < NSPLIT; ++q) {
-                const int row = row0 + q * ITS + (lu & (ITS - 1));
-                yv[q] = row < vt ? __ldg(p.Y + r0 + (long long)j * BT + row) : 0.f;
-            }
+            float ynext = 0.f;
+            if (yholder && yrow < nrows) ynext = __ldg(p.Y + nr0 + yrow);
 
             float hreg[ITER][4];
             float w2r[4];
@@ -228,7 +217,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                             *reinterpret_cast<const ulonglong2*>(W1s + (q * S + lu + u * LPS) * 4);
                         w[u][2 * q] = a.x; w[u][2 * q + 1] = a.y;
                     }
-                mbar_wait(bar_full + 8 * buf, ph);
+                mbar_wait(bar_full + 8 * xst, xph);
 #pragma unroll
                 for (int q = 0; q < NSPLIT; ++q) {
                     float pv[ITS];
@@ -269,65 +258,80 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                 }
             }
 
-            // ---------------- backward: eqs. 5-8 (the same registers now hold dW1) ----------------
-            // acc[AI(u, kk)] accumulates dW1 for unit u and the input pair (2kk, 2kk+1); the flat
-            // order is the one SubgroupReduce transposes (see AI below).
-            f32x2 acc[64];
-            auto AI = [](int u, int kk) constexpr -> int {
-                const int q = kk >> 1, hb = kk & 1, c2 = q / SPW, sp = q % SPW;
-                return SPW * ((u * CPL + c2) * 2 + hb) + sp;
-            };
+            // ---------------- backward: eqs. 5-8 ----------------
+            // K-split: the lane of sub-group s accumulates dW1 only for the IPS inputs
+            // [IPS*s, IPS*(s+1)) of its four units, but over the rows of ALL sub-groups, so no
+            // reduction across sub-groups is needed afterwards.  dZ1 of the other sub-groups'
+            // rows arrives by shuffle; acc[u][kk] <-> inputs IPS*s + 2kk, +1.
+            constexpr int IPS = kIn / SPW;            // inputs per sub-group
+            f32x2 acc[4][IPS / 2];
+            const float* Xk = Xs + xst * XSTAGE + rowl * kIn + IPS * s;
 #pragma unroll
             for (int q = 0; q < NSPLIT; ++q) {
-                mbar_wait_cluster(bar_yp + 8 * (buf * NSPLIT + q), ph);
+                // The partials were written by st.async, whose completion is the barrier's
+                // transaction count: the default (CTA-scope acquire) wait orders them; a
+                // cluster-scope acquire would make ptxas emit CCTL.IVALL (L1 invalidate), which
+                // stalls on every global load in flight.
+                mbar_wait(bar_yp + 8 * (buf * NSPLIT + q), ph);
                 float dzv;
                 {
-                    const int row = row0 + q * ITS + (lu & (ITS - 1));
+                    const int kk = lu & (ITS - 1);
+                    const int row = row0 + q * ITS + kk;
+                    const float yv = __shfl_sync(0xffffffffu, ycur, s * ITER + q * ITS + kk);
                     float yp = 0.f;
                     for (uint32_t c = 0; c < C; ++c) yp += ypt[c * BT + row];  // fixed rank order
-                    dzv = row < vt ? scale * (yp - yv[q]) : 0.f;              // eq. 5
+                    dzv = row < vt ? scale * (yp - yv) : 0.f;                 // eq. 5
                 }
 #pragma unroll
                 for (int k = 0; k < ITS; ++k) {
                     const int it = q * ITS + k;
                     const float d = __shfl_sync(0xffffffffu, dzv, (lane & ~(LPS - 1)) | k);
-                    f32x2 dd[4];
+                    float e[4];
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const float h = hreg[it][u];
                         g2[u] = fmaf(h, d, g2[u]);                             // eq. 6
-                        const float e = h > 0.f ? d * w2r[u] : 0.f;            // eq. 7 (old W2)
-                        dd[u] = pack2(e, e);
+                        e[u] = h > 0.f ? d * w2r[u] : 0.f;                     // eq. 7 (old W2)
                     }
-                    const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xl + it * kIn);
 #pragma unroll
-                    for (int x = 0; x < 8; ++x) {                              // eq. 8
-                        const ulonglong2 xv = xrow[x];
+                    for (int t = 0; t < SPW; ++t) {            // row of sub-group s ^ t
+                        f32x2 dd[4];
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
-                            if (it == 0) {
-                                acc[AI(u, 2 * x)] = fmul2(xv.x, dd[u]);
-                                acc[AI(u, 2 * x + 1)] = fmul2(xv.y, dd[u]);
-                            } else {
-                                ffma2(acc[AI(u, 2 * x)], xv.x, dd[u]);
-                                ffma2(acc[AI(u, 2 * x + 1)], xv.y, dd[u]);
+                            const float eo = t == 0 ? e[u] : __shfl_xor_sync(0xffffffffu, e[u], t * LPS);
+                            dd[u] = pack2(eo, eo);
+                        }
+                        const ulonglong2* xrow =
+                            reinterpret_cast<const ulonglong2*>(Xk + (s ^ t) * XBLK + it * kIn);
+#pragma unroll
+                        for (int x = 0; x < IPS / 4; ++x) {                    // eq. 8
+                            const ulonglong2 xv = xrow[x];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                if (it == 0 && t == 0) {
+                                    acc[u][2 * x] = fmul2(xv.x, dd[u]);
+                                    acc[u][2 * x + 1] = fmul2(xv.y, dd[u]);
+                                } else {
+                                    ffma2(acc[u][2 * x], xv.x, dd[u]);
+                                    ffma2(acc[u][2 * x + 1], xv.y, dd[u]);
+                                }
                             }
                         }
                     }
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * buf);   // this warp is done with the X tile
+            if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp is done with the X tile
+            ycur = ynext;
 
-            // combine the SPW sub-groups; lane (s, lu) ends with chunks q = SPW*c2 + s of its units
-            SubgroupReduce<64, SPW, LPS>::run(acc, s);
+            // lane (s, lu) owns the 4-input chunks q = (IPS/4)*s + x of its four units
 #pragma unroll
             for (int u = 0; u < 4; ++u)
 #pragma unroll
-                for (int c2 = 0; c2 < CPL; ++c2) {
-                    const int q = SPW * c2 + s;
+                for (int x = 0; x < IPS / 4; ++x) {
+                    const int q = (IPS / 4) * s + x;
                     ulonglong2* dst = reinterpret_cast<ulonglong2*>(mypart + (q * S + lu + u * LPS) * 4);
-                    f32x2 lo = acc[(u * CPL + c2) * 2], hi = acc[(u * CPL + c2) * 2 + 1];
+                    f32x2 lo = acc[u][2 * x], hi = acc[u][2 * x + 1];
                     if (j > 0) {                               // later tiles of a large batch
                         const ulonglong2 old = *dst;
                         lo = fadd2(lo, old.x); hi = fadd2(hi, old.y);
@@ -389,9 +393,9 @@ cudaError_t launch_cfg(const TrainParams& p, int cluster, cudaStream_t stream) {
     constexpr int ITER = BT / SPW / kWarps;
     constexpr int NSPLIT = ITER >= 2 ? 2 : 1;
     auto kern = k_train_fused<S, BT, NSPLIT>;
-    const size_t smem = sizeof(float) * (2 * (BT * kIn + SPW * 4) + 2 * cluster * BT +
+    const size_t smem = sizeof(float) * (kRing * (BT * kIn + SPW * 4) + 2 * cluster * BT +
                                          kWarps * S * kIn + kWarps * S + S * kIn + S) +
-                        8 * (4 + 2 * NSPLIT);
+                        8 * (2 * kRing + 2 * NSPLIT);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     if (cluster > 8) {
