@@ -149,6 +149,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     }
 
     const int rowl = warp * ITER;                     // first row of this lane inside its block
+    // Ypred exchange: every lane pushes to one fixed peer (staggered by rank)
+    const int cshift = __ffs((int)C) - 1;
+    const uint32_t pd = ((lane & (C - 1)) + crank) & (C - 1);
+    const uint32_t rem_ypp = mapa(smem_u32(ypp), pd), rem_bar = mapa(bar_yp, pd);
+    const int npush = (ITS * SPW * (int)C + 31) / 32;
     float* mypart = part + warp * (S * kIn);
     // Targets: lane l < ITER*SPW of a warp holds Y of the warp's row (l / ITER, l % ITER); it is
     // fetched one tile ahead (global-load latency hidden by a whole tile) and handed to the lane
@@ -246,13 +251,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                         pv[k] = pr;
                     }
                     GroupReduce<ITS, LPS>::run(pv, lu);
-                    if (lu < ITS) {
-                        const int row = row0 + q * ITS + lu;
-                        const uint32_t dst = smem_u32(ypp + buf * (C * BT) + crank * BT + row);
-                        const uint32_t bar = bar_yp + 8 * (buf * NSPLIT + q);
-                        for (uint32_t dd = 0; dd < C; ++dd) {
-                            const uint32_t d = (crank + dd) % C;
-                            st_async_f32(mapa(dst, d), pv[0], mapa(bar, d));
+                    // push: lane l serves ONE destination CTA (pd) and the rows l/C, l/C + 32/C, ...
+                    // of the warp's ITS*SPW totals, fetched from their holder lanes by shuffle
+#pragma unroll 1
+                    for (int i = 0; i < npush; ++i) {
+                        const int r = (lane >> cshift) + i * (32 >> cshift);
+                        const int sp = r / ITS, k = r % ITS;
+                        const float v = __shfl_sync(0xffffffffu, pv[0], (sp * LPS + k) & 31);
+                        if (r < ITS * SPW) {
+                            const int row = sp * RB + rowl + q * ITS + k;
+                            st_async_f32(rem_ypp + (buf * (C * BT) + crank * BT + row) * 4, v,
+                                         rem_bar + 8 * (buf * NSPLIT + q));
                         }
                     }
                 }
