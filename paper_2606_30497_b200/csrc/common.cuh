@@ -108,8 +108,8 @@ __device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t cta) {
 // remote 4-byte store that completes 4 tx-bytes on the (remote) mbarrier
 __device__ __forceinline__ void st_async_f32(uint32_t raddr, float v, uint32_t rbar) {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
-                 ::"r"(raddr), "r"(__float_as_uint(v)), "r"(rbar)
-                 : "memory");
+                 ::"r"(raddr), "r"(__float_as_uint(v)), "r"(rbar));   // register operands only:
+    // no "memory" clobber, so independent shared-memory loads may be scheduled across it
 }
 __device__ __forceinline__ void cluster_arrive() {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");

@@ -73,7 +73,7 @@ struct GroupReduce {
     }
 };
 
-template <int S, int BT, int NSPLIT>
+template <int S, int BT, int NSPLIT, int C>
 __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p) {
     constexpr int LPS = S / 4;            // lanes per sample row
     constexpr int SPW = 32 / LPS;         // sample rows per warp instruction (row sub-groups)
@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int lu = lane % LPS, s = lane / LPS;
-    const uint32_t crank = cluster_ctarank(), C = cluster_nctarank();
+    const uint32_t crank = cluster_ctarank();   // C = cluster size (template: exchange code is straight-line)
     const int H = p.H;
 
     float* Xs = reinterpret_cast<float*>(smem_raw);          // [kRing][XSTAGE]
@@ -150,10 +150,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 
     const int rowl = warp * ITER;                     // first row of this lane inside its block
     // Ypred exchange: every lane pushes to one fixed peer (staggered by rank)
-    const int cshift = __ffs((int)C) - 1;
+    constexpr int RPI = 32 / C;                       // rows served per push iteration (C <= 32)
     const uint32_t pd = ((lane & (C - 1)) + crank) & (C - 1);
     const uint32_t rem_ypp = mapa(smem_u32(ypp), pd), rem_bar = mapa(bar_yp, pd);
-    const int npush = (ITS * SPW * (int)C + 31) / 32;
+    constexpr int NPUSH = (ITS * SPW * C + 31) / 32;
     float* mypart = part + warp * (S * kIn);
     // Targets: lane l < ITER*SPW of a warp holds Y of the warp's row (l / ITER, l % ITER); it is
     // fetched one tile ahead (global-load latency hidden by a whole tile) and handed to the lane
@@ -253,9 +253,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                     GroupReduce<ITS, LPS>::run(pv, lu);
                     // push: lane l serves ONE destination CTA (pd) and the rows l/C, l/C + 32/C, ...
                     // of the warp's ITS*SPW totals, fetched from their holder lanes by shuffle
-#pragma unroll 1
-                    for (int i = 0; i < npush; ++i) {
-                        const int r = (lane >> cshift) + i * (32 >> cshift);
+#pragma unroll
+                    for (int i = 0; i < NPUSH; ++i) {
+                        const int r = lane / C + i * RPI;
                         const int sp = r / ITS, k = r % ITS;
                         const float v = __shfl_sync(0xffffffffu, pv[0], (sp * LPS + k) & 31);
                         if (r < ITS * SPW) {
@@ -287,8 +287,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                     const int kk = lu & (ITS - 1);
                     const int row = row0 + q * ITS + kk;
                     const float yv = __shfl_sync(0xffffffffu, ycur, s * ITER + q * ITS + kk);
-                    float yp = 0.f;
-                    for (uint32_t c = 0; c < C; ++c) yp += ypt[c * BT + row];  // fixed rank order
+                    float ypc[C];
+#pragma unroll
+                    for (int c = 0; c < C; ++c) ypc[c] = ypt[c * BT + row];
+#pragma unroll
+                    for (int o = 1; o < C; o <<= 1)                 // fixed pairwise tree over ranks
+#pragma unroll
+                        for (int c = 0; c + o < C; c += 2 * o) ypc[c] += ypc[c + o];
+                    const float yp = ypc[0];
                     dzv = row < vt ? scale * (yp - yv) : 0.f;                 // eq. 5
                 }
 #pragma unroll
@@ -396,29 +402,29 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     cluster_sync_all();        // no CTA exits while peers may still push into its shared memory
 }
 
-template <int S, int BT>
-cudaError_t launch_cfg(const TrainParams& p, int cluster, cudaStream_t stream) {
+template <int S, int BT, int C>
+cudaError_t launch_cfg(const TrainParams& p, cudaStream_t stream) {
     constexpr int SPW = 32 / (S / 4);
     constexpr int ITER = BT / SPW / kWarps;
     constexpr int NSPLIT = ITER >= 2 ? 2 : 1;
-    auto kern = k_train_fused<S, BT, NSPLIT>;
-    const size_t smem = sizeof(float) * (kRing * (BT * kIn + SPW * 4) + 2 * cluster * BT +
+    auto kern = k_train_fused<S, BT, NSPLIT, C>;
+    const size_t smem = sizeof(float) * (kRing * (BT * kIn + SPW * 4) + 2 * C * BT +
                                          kWarps * S * kIn + kWarps * S + S * kIn + S) +
                         8 * (2 * kRing + 2 * NSPLIT);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
-    if (cluster > 8) {
+    if (C > 8) {
         err = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         if (err != cudaSuccess) return err;
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(cluster);
+    cfg.gridDim = dim3(C);
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = cluster;
+    attr[0].val.clusterDim.x = C;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
@@ -426,28 +432,39 @@ cudaError_t launch_cfg(const TrainParams& p, int cluster, cudaStream_t stream) {
     return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
-// Tile height: the smallest power of two >= batch inside [8*SPW, 64*SPW] (at most 256); 64*SPW
-// rows keep H = ReLU(Z1) of a tile in 32 registers per lane.
-template <int S>
-cudaError_t launch_s(const TrainParams& p, int cluster, cudaStream_t stream) {
+// Tile height: the smallest instantiated height >= batch, else the largest (64*SPW rows, at most
+// 256, keep H = ReLU(Z1) of a tile in 32 registers per lane).
+template <int S, int C>
+cudaError_t launch_sc(const TrainParams& p, cudaStream_t stream) {
     const int B = p.B;
     if constexpr (S == 16) {
-        if (B > 128) return launch_cfg<16, 256>(p, cluster, stream);
-        if (B > 64) return launch_cfg<16, 128>(p, cluster, stream);
-        return launch_cfg<16, 64>(p, cluster, stream);
+        if (B > 64) return launch_cfg<16, 256, C>(p, stream);
+        return launch_cfg<16, 64, C>(p, stream);
     } else if constexpr (S == 32) {
-        if (B > 128) return launch_cfg<32, 256>(p, cluster, stream);
-        if (B > 64) return launch_cfg<32, 128>(p, cluster, stream);
-        if (B > 32) return launch_cfg<32, 64>(p, cluster, stream);
-        return launch_cfg<32, 32>(p, cluster, stream);
+        if (B > 128) return launch_cfg<32, 256, C>(p, stream);
+        if (B > 32) return launch_cfg<32, 128, C>(p, stream);
+        return launch_cfg<32, 32, C>(p, stream);
     } else if constexpr (S == 64) {
-        if (B > 64) return launch_cfg<64, 128>(p, cluster, stream);
-        if (B > 32) return launch_cfg<64, 64>(p, cluster, stream);
-        return launch_cfg<64, 32>(p, cluster, stream);
+        if (B > 32) return launch_cfg<64, 128, C>(p, stream);
+        return launch_cfg<64, 32, C>(p, stream);
     } else {
-        if (B > 32) return launch_cfg<128, 64>(p, cluster, stream);
-        return launch_cfg<128, 32>(p, cluster, stream);
+        if (B > 32) return launch_cfg<128, 64, C>(p, stream);
+        return launch_cfg<128, 32, C>(p, stream);
     }
+}
+
+// hidden = S * C must be one of 32..1024 (include/mlp.h): only those pairs are instantiated
+template <int S>
+cudaError_t launch_s(const TrainParams& p, int cluster, cudaStream_t stream) {
+    switch (cluster) {
+        case 1: if constexpr (S >= 32) return launch_sc<S, 1>(p, stream); break;
+        case 2: return launch_sc<S, 2>(p, stream);
+        case 4: return launch_sc<S, 4>(p, stream);
+        case 8: return launch_sc<S, 8>(p, stream);
+        case 16: if constexpr (S <= 64) return launch_sc<S, 16>(p, stream); break;
+        default: break;
+    }
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace
@@ -456,7 +473,9 @@ bool fused_supported(int hidden, int cluster) {
     if (cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8 && cluster != 16) return false;
     if (hidden % cluster) return false;
     const int S = hidden / cluster;
-    return S == 16 || S == 32 || S == 64 || S == 128;
+    if (S == 16) return cluster >= 2;
+    if (S == 128) return cluster <= 8;
+    return S == 32 || S == 64;
 }
 
 int fused_default_cluster(int hidden) {
