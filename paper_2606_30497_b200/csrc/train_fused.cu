@@ -241,14 +241,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                                 ffma2(a[u], xv.y, w[u][2 * x + 1]);
                             }
                         }
-                        float pr = 0.f;
 #pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const float h = fmaxf(hsum2(a[u]), 0.f);                     // eq. 2
-                            hreg[it][u] = h;
-                            pr = fmaf(h, w2r[u], pr);                                    // eq. 3
-                        }
-                        pv[k] = pr;
+                        for (int u = 0; u < 4; ++u) hreg[it][u] = fmaxf(hsum2(a[u]), 0.f);   // eq. 2
+                        pv[k] = fmaf(hreg[it][1], w2r[1], hreg[it][0] * w2r[0]) +            // eq. 3
+                                fmaf(hreg[it][3], w2r[3], hreg[it][2] * w2r[2]);
                     }
                     GroupReduce<ITS, LPS>::run(pv, lu);
                     // push: lane l serves ONE destination CTA (pd) and the rows l/C, l/C + 32/C, ...
@@ -365,16 +361,30 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             for (int u = 0; u < 4; ++u) part2[warp * S + lu + u * LPS] = g2[u];
         }
         __syncthreads();
-        for (int f = tid; f < S * 8; f += kThreads) {
-            float4 sum = reinterpret_cast<const float4*>(part)[f];
+        {
+            constexpr int NF = S * 8;                          // float4 slots of this CTA's dW1
+            const f32x2 nlr2 = pack2(-p.lr, -p.lr);
 #pragma unroll
-            for (int w = 1; w < kWarps; ++w) {
-                const float4 v = reinterpret_cast<const float4*>(part)[w * S * 8 + f];
-                sum.x += v.x; sum.y += v.y; sum.z += v.z; sum.w += v.w;
+            for (int r = 0; r < (NF + kThreads - 1) / kThreads; ++r) {
+                const int f = tid + r * kThreads;
+                if (NF % kThreads == 0 || f < NF) {
+                    ulonglong2 v[kWarps];
+#pragma unroll
+                    for (int w = 0; w < kWarps; ++w)
+                        v[w] = reinterpret_cast<const ulonglong2*>(part)[w * NF + f];
+#pragma unroll
+                    for (int o = 1; o < kWarps; o <<= 1)        // fixed pairwise tree over warps
+#pragma unroll
+                        for (int w = 0; w + o < kWarps; w += 2 * o) {
+                            v[w].x = fadd2(v[w].x, v[w + o].x);
+                            v[w].y = fadd2(v[w].y, v[w + o].y);
+                        }
+                    ulonglong2 wv = reinterpret_cast<ulonglong2*>(W1s)[f];
+                    ffma2(wv.x, v[0].x, nlr2);                                 // eq. 9: W - lr*dW
+                    ffma2(wv.y, v[0].y, nlr2);
+                    reinterpret_cast<ulonglong2*>(W1s)[f] = wv;
+                }
             }
-            float4 wv = reinterpret_cast<float4*>(W1s)[f];
-            wv.x -= p.lr * sum.x; wv.y -= p.lr * sum.y; wv.z -= p.lr * sum.z; wv.w -= p.lr * sum.w;
-            reinterpret_cast<float4*>(W1s)[f] = wv;                            // eq. 9
         }
         if (tid < S) {
             float sum = part2[tid];
