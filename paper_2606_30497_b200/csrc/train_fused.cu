@@ -92,7 +92,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     const int H = p.H;
 
     float* Xs = reinterpret_cast<float*>(smem_raw);          // [kRing][XSTAGE]
-    float* ypp = Xs + kRing * XSTAGE;                         // [2][C][BT]
+    constexpr int XRING = (kRing * XSTAGE + 31) / 32 * 32;    // floats; keeps what follows 128-byte aligned
+    float* ypp = Xs + XRING;                                  // [2][C][BT]
     float* part = ypp + 2 * C * BT;                           // [kWarps][S*32]  layout [q][u][4]
     float* part2 = part + kWarps * S * kIn;                   // [kWarps][S]
     float* W1s = part2 + kWarps * S;                          // [S*32]          layout [q][u][4]
@@ -418,7 +419,7 @@ cudaError_t launch_cfg(const TrainParams& p, cudaStream_t stream) {
     constexpr int ITER = BT / SPW / kWarps;
     constexpr int NSPLIT = ITER >= 2 ? 2 : 1;
     auto kern = k_train_fused<S, BT, NSPLIT, C>;
-    const size_t smem = sizeof(float) * (kRing * (BT * kIn + SPW * 4) + 2 * C * BT +
+    const size_t smem = sizeof(float) * ((kRing * (BT * kIn + SPW * 4) + 31) / 32 * 32 + 2 * C * BT +
                                          kWarps * S * kIn + kWarps * S + S * kIn + S) +
                         8 * (2 * kRing + 2 * NSPLIT);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
