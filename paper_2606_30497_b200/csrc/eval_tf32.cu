@@ -80,10 +80,8 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
             double* __restrict__ partials, unsigned int* __restrict__ ticket,
             double* __restrict__ out) {
     static_assert(H % 32 == 0 && H >= 32 && H <= 256, "one MMA N-extent, 32-column TMEM loads");
-    extern __shared__ unsigned char smem_dyn[];
-    // 1024-byte alignment: swizzle atoms of both operands
-    unsigned char* smem = reinterpret_cast<unsigned char*>(
-        (reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~static_cast<uintptr_t>(1023));
+    // 1024-byte alignment: swizzle atoms of both operands (checked below)
+    extern __shared__ __align__(1024) unsigned char smem[];
     float* Bs = reinterpret_cast<float*>(smem);                            // [H][32] swizzled
     unsigned char* Xring = smem + H * kIn * 4;                             // [kStages][16 KB]
     float* W2s = reinterpret_cast<float*>(Xring + kStages * kTileBytes);   // [H]
@@ -117,6 +115,7 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    if (smem_u32(smem) & 1023u) __trap();
 
     const long long ntiles = (n + kTile - 1) / kTile;
     const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -157,6 +156,7 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     } else {
         // ===== epilogue: set e handles tiles i with (i & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
         const int e = (warp - 2) >> 2, q = warp & 3;
+        float sse32 = 0.f;
         for (long long i = e; i < my_tiles; i += 2) {
             const long long row = (blockIdx.x + i * (long long)gridDim.x) * kTile + q * 32 + lane;
             const float yv = row < n ? __ldg(Y + row) : 0.f;
@@ -188,11 +188,11 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
                 }
             }
             const float yp = (hsum2(acc[0]) + hsum2(acc[1])) + (hsum2(acc[2]) + hsum2(acc[3]));
-            if (row < n) {
-                const float err = yp - yv;
-                sse += (double)(err * err);                                    // eq. 4
-            }
+            const float err = row < n ? yp - yv : 0.f;
+            sse32 = fmaf(err, err, sse32);                                     // eq. 4
+            if (((i >> 1) & 31) == 31) { sse += (double)sse32; sse32 = 0.f; }  // fp64 every 32 tiles
         }
+        sse += (double)sse32;
         for (int o = 16; o > 0; o >>= 1) sse += __shfl_down_sync(0xffffffffu, sse, o);
         if (lane == 0) wsum[warp - 2] = sse;
     }
@@ -243,7 +243,7 @@ template <int H>
 cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const float* W1, const float* W2,
                      double* partials, int grid, double* d_out, cudaStream_t stream) {
     auto kern = k_eval_tf32<H>;
-    const size_t smem = 1024 + (size_t)H * kIn * 4 + (size_t)kStages * kTileBytes + (size_t)H * 4 +
+    const size_t smem = (size_t)H * kIn * 4 + (size_t)kStages * kTileBytes + (size_t)H * 4 +
                         8 * (2 * kStages + 4) + 8 * 8 + 16;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
