@@ -68,6 +68,16 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// one lane of a converged warp (the MMA / TMA issue must not sit behind a divergent branch: UTCHMMA
+// and UTMALDG take uniform registers, and ptxas wraps them in per-lane loops otherwise)
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred = 0;
+    asm volatile(
+        "{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 // K-major, 128-byte-swizzled operand descriptor (8-row x 128-byte atoms, 1024 bytes apart)
 __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
@@ -80,16 +90,20 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
             double* __restrict__ partials, unsigned int* __restrict__ ticket,
             double* __restrict__ out) {
     static_assert(H % 32 == 0 && H >= 32 && H <= 256, "one MMA N-extent, 32-column TMEM loads");
+    // Each 256-column TMEM accumulator is filled and drained in NH column parts, so the MMA of the
+    // next tile's first part overlaps the epilogue of this tile's second part.
+    constexpr int NH = H >= 128 ? 2 : 1;
+    constexpr int CP = H / NH;                 // columns (hidden units) per part
     // 1024-byte alignment: swizzle atoms of both operands (checked below)
     extern __shared__ __align__(1024) unsigned char smem[];
     float* Bs = reinterpret_cast<float*>(smem);                            // [H][32] swizzled
     unsigned char* Xring = smem + H * kIn * 4;                             // [kStages][16 KB]
     float* W2s = reinterpret_cast<float*>(Xring + kStages * kTileBytes);   // [H]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + H);                 // full, empty, tfull[2], tempty[2]
-    double* wsum = reinterpret_cast<double*>(bars + 2 * kStages + 4);      // [8]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + H);                 // full, empty, tfull[2][2], tempty[2][2]
+    double* wsum = reinterpret_cast<double*>(bars + 2 * kStages + 8);      // [8]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(wsum + 8);
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kStages),
-                   bar_tfull = smem_u32(bars + 2 * kStages), bar_tempty = smem_u32(bars + 2 * kStages + 2);
+                   bar_tfull = smem_u32(bars + 2 * kStages), bar_tempty = smem_u32(bars + 2 * kStages + 4);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
@@ -99,10 +113,11 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
         const int off = (j >> 3) * 1024 + (j & 7) * 128 + ((((k >> 2) ^ (j & 7)) << 4) | ((k & 3) << 2));
         *reinterpret_cast<float*>(smem + off) = W1[(size_t)k * H + j];
     }
-    for (int j = tid; j < H; j += kEvalThreads) W2s[j] = W2[j];
+    // columns 24..31 of every 32 take ReLU as (z + |z|) on the FMA pipe: their W2 carries the 1/2
+    for (int j = tid; j < H; j += kEvalThreads) W2s[j] = (j & 31) >= 24 ? 0.5f * W2[j] : W2[j];
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
+        for (int b = 0; b < 4; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -121,70 +136,86 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     double sse = 0.0;
 
+    const uint32_t nt = (uint32_t)my_tiles;
     if (warp == 0) {
-        // ===== TMA producer =====
-        if (lane == 0) {
-            for (long long i = 0; i < my_tiles; ++i) {
-                const int st = (int)(i % kStages);
-                if (i >= kStages) mbar_wait(bar_empty + 8 * st, (unsigned)((i / kStages) - 1) & 1u);
-                const long long row0 = (blockIdx.x + i * (long long)gridDim.x) * kTile;
+        // ===== TMA producer (whole warp runs the loop, one elected lane issues) =====
+        uint32_t st = 0, eph = 1;                       // ring stage, parity of the "empty" phase to wait for
+        for (uint32_t i = 0; i < nt; ++i) {
+            if (i >= kStages) mbar_wait(bar_empty + 8 * st, eph);
+            if (elect_one()) {
+                const long long row0 = (blockIdx.x + (long long)i * gridDim.x) * kTile;
                 mbar_arrive_expect_tx(bar_full + 8 * st, kTileBytes);   // OOB rows are zero-filled, still counted
-                tma_load_2d(smem_u32(Xring + st * kTileBytes), &tmapX, 0, (int)row0, bar_full + 8 * st);
+                tma_load_2d(smem_u32(Xring) + st * kTileBytes, &tmapX, 0, (int)row0, bar_full + 8 * st);
             }
+            __syncwarp();
+            if (++st == kStages) { st = 0; eph ^= 1u; }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer (one thread) =====
-        if (lane == 0) {
-            // instruction descriptor: D=f32, A=B=tf32, both K-major, N=H, M=128
-            constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(H >> 3) << 17) |
-                                       ((uint32_t)(kTile >> 4) << 24);
-            const uint64_t bdesc = smem_desc_sw128(smem_u32(Bs));
-            for (long long i = 0; i < my_tiles; ++i) {
-                const int st = (int)(i % kStages);
-                const unsigned b = (unsigned)(i & 1);
-                if (i >= 2) mbar_wait(bar_tempty + 8 * b, (unsigned)((i >> 1) - 1) & 1u);
-                mbar_wait(bar_full + 8 * st, (unsigned)(i / kStages) & 1u);
-                tc_fence_after();
-                const uint64_t adesc = smem_desc_sw128(smem_u32(Xring + st * kTileBytes));
+        // ===== MMA issuer (whole warp runs the loop, one elected lane issues) =====
+        // instruction descriptor: D=f32, A=B=tf32, both K-major, N=CP, M=128
+        constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(CP >> 3) << 17) |
+                                   ((uint32_t)(kTile >> 4) << 24);
+        const uint64_t bdesc = smem_desc_sw128(smem_u32(Bs));
+        const uint64_t adesc0 = smem_desc_sw128(smem_u32(Xring));
+        uint32_t st = 0, fph = 0;
+        for (uint32_t i = 0; i < nt; ++i) {
+            const uint32_t b = i & 1u, tph = ((i >> 1) - 1u) & 1u;
+            mbar_wait(bar_full + 8 * st, fph);
+            const uint64_t adesc = adesc0 + (uint64_t)(st * (kTileBytes >> 4));
 #pragma unroll
-                for (int k = 0; k < kIn / 8; ++k)      // K = 8 tf32 = 32 bytes per MMA: +2 in 16-byte units
-                    mma_tf32(tmem_base + b * 256, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
-                tc_commit(bar_empty + 8 * st);          // ring slot free once these MMAs have read it
-                tc_commit(bar_tfull + 8 * b);           // accumulator ready
+            for (int hf = 0; hf < NH; ++hf) {
+                if (i >= 2) mbar_wait(bar_tempty + 8 * (2 * b + hf), tph);
+                tc_fence_after();
+                if (elect_one()) {
+#pragma unroll
+                    for (int k = 0; k < kIn / 8; ++k)  // K = 8 tf32 = 32 bytes per MMA: +2 in 16-byte units
+                        mma_tf32(tmem_base + b * 256 + hf * CP, adesc + 2 * k,
+                                 bdesc + (uint64_t)(hf * CP * 128 / 16) + 2 * k, idesc, k > 0);
+                    if (hf == NH - 1) tc_commit(bar_empty + 8 * st);   // ring slot free once read
+                    tc_commit(bar_tfull + 8 * (2 * b + hf));           // accumulator part ready
+                }
+                __syncwarp();
             }
+            if (++st == kStages) { st = 0; fph ^= 1u; }
         }
     } else {
         // ===== epilogue: set e handles tiles i with (i & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
         const int e = (warp - 2) >> 2, q = warp & 3;
         float sse32 = 0.f;
-        for (long long i = e; i < my_tiles; i += 2) {
-            const long long row = (blockIdx.x + i * (long long)gridDim.x) * kTile + q * 32 + lane;
+        for (uint32_t i = e; i < nt; i += 2) {
+            const long long row = (blockIdx.x + (long long)i * gridDim.x) * kTile + q * 32 + lane;
             const float yv = row < n ? __ldg(Y + row) : 0.f;
-            mbar_wait(bar_tfull + 8 * e, (unsigned)(i >> 1) & 1u);
-            tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + e * 256;
-            uint32_t z[2][32];
             f32x2 acc[4] = {0ull, 0ull, 0ull, 0ull};
-            tmem_ld32(taddr, z[0]);
-            tmem_ld_wait();
 #pragma unroll
-            for (int c = 0; c < H / 32; ++c) {
-                if (c + 1 < H / 32) tmem_ld32(taddr + (c + 1) * 32, z[(c + 1) & 1]);
+            for (int hf = 0; hf < NH; ++hf) {
+                mbar_wait(bar_tfull + 8 * (2 * e + hf), (unsigned)(i >> 1) & 1u);
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + e * 256 + hf * CP;
+                uint32_t z[2][32];
+                tmem_ld32(taddr, z[0]);
+                tmem_ld_wait();
 #pragma unroll
-                for (int g = 0; g < 8; ++g) {                                  // 4 columns per W2 load
-                    const ulonglong2 w = *reinterpret_cast<const ulonglong2*>(W2s + c * 32 + g * 4);
-                    const uint32_t* zz = z[c & 1] + g * 4;
-                    const f32x2 h01 = pack2(fmaxf(__uint_as_float(zz[0]), 0.f), fmaxf(__uint_as_float(zz[1]), 0.f));
-                    const f32x2 h23 = pack2(fmaxf(__uint_as_float(zz[2]), 0.f), fmaxf(__uint_as_float(zz[3]), 0.f));
-                    ffma2(acc[(2 * g) & 3], h01, w.x);                         // eqs. 2-3
-                    ffma2(acc[(2 * g + 1) & 3], h23, w.y);
-                }
-                if (c + 1 < H / 32) tmem_ld_wait();
-                if (c + 2 == H / 32 || H == 32) {
-                    // every column of this accumulator is now in registers: hand it back to the MMA warp
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar_tempty + 8 * e);
+                for (int c = 0; c < CP / 32; ++c) {
+                    if (c + 1 < CP / 32) tmem_ld32(taddr + (c + 1) * 32, z[(c + 1) & 1]);
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {                              // 4 columns per W2 load
+                        const ulonglong2 w = *reinterpret_cast<const ulonglong2*>(W2s + hf * CP + c * 32 + g * 4);
+                        float h[4];
+#pragma unroll
+                        for (int t = 0; t < 4; ++t) {
+                            const float zz = __uint_as_float(z[c & 1][g * 4 + t]);
+                            h[t] = g < 6 ? fmaxf(zz, 0.f) : zz + fabsf(zz);     // eq. 2 (ALU pipe / FMA pipe)
+                        }
+                        ffma2(acc[(2 * g) & 3], pack2(h[0], h[1]), w.x);       // eq. 3
+                        ffma2(acc[(2 * g + 1) & 3], pack2(h[2], h[3]), w.y);
+                    }
+                    if (c + 1 < CP / 32) tmem_ld_wait();
+                    if (c + 2 == CP / 32 || CP == 32) {
+                        // every column of this part is now in registers: hand it back to the MMA warp
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_tempty + 8 * (2 * e + hf));
+                    }
                 }
             }
             const float yp = (hsum2(acc[0]) + hsum2(acc[1])) + (hsum2(acc[2]) + hsum2(acc[3]));
@@ -244,7 +275,7 @@ cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const
                      double* partials, int grid, double* d_out, cudaStream_t stream) {
     auto kern = k_eval_tf32<H>;
     const size_t smem = (size_t)H * kIn * 4 + (size_t)kStages * kTileBytes + (size_t)H * 4 +
-                        8 * (2 * kStages + 4) + 8 * 8 + 16;
+                        8 * (2 * kStages + 8) + 8 * 8 + 16;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     unsigned int* ticket = reinterpret_cast<unsigned int*>(partials + grid);
