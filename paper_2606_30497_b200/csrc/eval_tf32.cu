@@ -9,14 +9,15 @@
 // Persistent grid, one CTA per SM, warp-specialised:
 //   warp 0      TMA producer: 128-row X tiles (16 KB) by cp.async.bulk.tensor with the 128-byte
 //               swizzle the MMA wants, into a kStages-deep ring;
-//   warp 1      MMA issuer: per tile four tcgen05.mma (M=128, N=hidden, K=8) into one of two
-//               TMEM accumulators (2 x 256 columns = all of TMEM); tcgen05.commit releases the
-//               ring slot and publishes the accumulator;
+//   warp 1      MMA issuer: per tile and column part four tcgen05.mma (M=128, N=hidden/NH, K=8)
+//               into one of two TMEM accumulators (2 x 256 columns = all of TMEM);
+//               tcgen05.commit releases the ring slot and publishes the accumulator part;
 //   warps 2-9   epilogue, two sets of four warps (even / odd tiles, one TMEM accumulator each):
 //               a thread owns one row, streams its hidden row out of TMEM (tcgen05.ld 32x32b),
-//               applies eq. 2-3 (max, FFMA2 with W2 broadcast from shared memory), eq. 4 in
-//               fp64.  Deterministic: fixed-order block and last-block reductions.
-// W1 is transposed once per CTA into the K-major swizzled B operand ([hidden][32] floats).
+//               applies eqs. 2-3 (ReLU + signed sum: |W2| is folded into the B operand, see
+//               "setup"), eq. 4 in compensated fp32 per thread, fp64 from the warp level up.
+//               Deterministic: fixed-order block and last-block reductions.
+// W1 diag|W2| is transposed once per CTA into the K-major swizzled B operand ([hidden][32] floats).
 #include <cuda.h>
 
 #include "common.cuh"
@@ -99,25 +100,50 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     float* Bs = reinterpret_cast<float*>(smem);                            // [H][32] swizzled
     unsigned char* Xring = smem + H * kIn * 4;                             // [kStages][16 KB]
     float* W2s = reinterpret_cast<float*>(Xring + kStages * kTileBytes);   // [H]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + H);                 // full, empty, tfull[2][2], tempty[2][2]
-    double* wsum = reinterpret_cast<double*>(bars + 2 * kStages + 8);      // [8]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(wsum + 8);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + H);                 // full, empty, tfull[2][NH], tempty[2][NH]
+    double* wsum = reinterpret_cast<double*>(bars + 2 * kStages + 16);      // [8]
+    int* colmap = reinterpret_cast<int*>(wsum + 8);                        // [H] permuted column of unit j
+    int* wcnt = colmap + H;                                                // [8]
+    int* npos_s = wcnt + 8;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(npos_s + 1);
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kStages),
-                   bar_tfull = smem_u32(bars + 2 * kStages), bar_tempty = smem_u32(bars + 2 * kStages + 4);
+                   bar_tfull = smem_u32(bars + 2 * kStages), bar_tempty = smem_u32(bars + 2 * kStages + 8);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
-    // ---- setup: B operand = W1^T (K-major, 128B swizzle), W2, barriers, TMEM ---------------------
-    for (int idx = tid; idx < H * kIn; idx += kEvalThreads) {
-        const int j = idx % H, k = idx / H;                                 // coalesced over j
-        const int off = (j >> 3) * 1024 + (j & 7) * 128 + ((((k >> 2) ^ (j & 7)) << 4) | ((k & 3) << 2));
-        *reinterpret_cast<float*>(smem + off) = W1[(size_t)k * H + j];
+    // ---- setup -------------------------------------------------------------------------------------
+    // W2 is folded into the B operand: column j of Z' = X (W1 diag|W2|) is |w2_j| z_j, and
+    //   w2_j ReLU(z_j) = sign(w2_j) ReLU(z'_j),
+    // so the epilogue needs no multiply and no W2 operand (the W2 loads used to take as many
+    // shared-memory cycles as the MMA operand reads).  Hidden units are permuted so that the
+    // npos units with w2 >= 0 come first: a 32-column chunk then has one sign, except the chunk
+    // holding column npos, which is corrected with 0/1 masks kept in registers.  Columns 24..31
+    // of every chunk take ReLU as (z + |z|) on the FMA pipe and carry a factor 1/2.
+    {
+        const bool mine = tid < H;
+        const float w2v = mine ? W2[tid] : -1.f;
+        const unsigned bal = __ballot_sync(0xffffffffu, mine && w2v >= 0.f);
+        if (mine && lane == 0) wcnt[warp] = __popc(bal);
+        __syncthreads();
+        if (mine) {
+            int before = __popc(bal & ((1u << lane) - 1u)), total = 0;
+            for (int w = 0; w < H / 32; ++w) { const int c = wcnt[w]; total += c; if (w < warp) before += c; }
+            const int dest = w2v >= 0.f ? before : total + (tid - before);
+            colmap[tid] = dest;
+            W2s[tid] = ((dest & 31) >= 24 ? 0.5f : 1.0f) * fabsf(w2v);
+            if (tid == 0) *npos_s = total;
+        }
+        __syncthreads();
     }
-    // columns 24..31 of every 32 take ReLU as (z + |z|) on the FMA pipe: their W2 carries the 1/2
-    for (int j = tid; j < H; j += kEvalThreads) W2s[j] = (j & 31) >= 24 ? 0.5f * W2[j] : W2[j];
+    for (int idx = tid; idx < H * kIn; idx += kEvalThreads) {
+        const int j0 = idx % H, k = idx / H;                                // coalesced over j0
+        const int j = colmap[j0];                                           // permuted column = B row
+        const int off = (j >> 3) * 1024 + (j & 7) * 128 + ((((k >> 2) ^ (j & 7)) << 4) | ((k & 3) << 2));
+        *reinterpret_cast<float*>(smem + off) = W1[(size_t)k * H + j0] * W2s[j0];
+    }
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
-        for (int b = 0; b < 4; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
+        for (int b = 0; b < 8; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -130,6 +156,7 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    const int npos = *npos_s;
     if (smem_u32(smem) & 1023u) __trap();
 
     const long long ntiles = (n + kTile - 1) / kTile;
@@ -164,7 +191,7 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
             const uint64_t adesc = adesc0 + (uint64_t)(st * (kTileBytes >> 4));
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) {
-                if (i >= 2) mbar_wait(bar_tempty + 8 * (2 * b + hf), tph);
+                if (i >= 2) mbar_wait(bar_tempty + 8 * (NH * b + hf), tph);
                 tc_fence_after();
                 if (elect_one()) {
 #pragma unroll
@@ -172,7 +199,7 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
                         mma_tf32(tmem_base + b * 256 + hf * CP, adesc + 2 * k,
                                  bdesc + (uint64_t)(hf * CP * 128 / 16) + 2 * k, idesc, k > 0);
                     if (hf == NH - 1) tc_commit(bar_empty + 8 * st);   // ring slot free once read
-                    tc_commit(bar_tfull + 8 * (2 * b + hf));           // accumulator part ready
+                    tc_commit(bar_tfull + 8 * (NH * b + hf));           // accumulator part ready
                 }
                 __syncwarp();
             }
@@ -181,14 +208,18 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     } else {
         // ===== epilogue: set e handles tiles i with (i & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
         const int e = (warp - 2) >> 2, q = warp & 3;
-        float sse32 = 0.f;
+        float sse32 = 0.f, comp = 0.f;
+        f32x2 negmask[16];                               // 1 for the w2 < 0 columns of the mixed chunk
+#pragma unroll
+        for (int t = 0; t < 16; ++t)
+            negmask[t] = pack2((2 * t) >= (npos & 31) ? 1.f : 0.f, (2 * t + 1) >= (npos & 31) ? 1.f : 0.f);
         for (uint32_t i = e; i < nt; i += 2) {
             const long long row = (blockIdx.x + (long long)i * gridDim.x) * kTile + q * 32 + lane;
             const float yv = row < n ? __ldg(Y + row) : 0.f;
-            f32x2 acc[4] = {0ull, 0ull, 0ull, 0ull};
+            float yp = 0.f;
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) {
-                mbar_wait(bar_tfull + 8 * (2 * e + hf), (unsigned)(i >> 1) & 1u);
+                mbar_wait(bar_tfull + 8 * (NH * e + hf), (unsigned)(i >> 1) & 1u);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + e * 256 + hf * CP;
                 uint32_t z[2][32];
@@ -197,33 +228,44 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
 #pragma unroll
                 for (int c = 0; c < CP / 32; ++c) {
                     if (c + 1 < CP / 32) tmem_ld32(taddr + (c + 1) * 32, z[(c + 1) & 1]);
+                    const int cb = hf * CP + c * 32;                            // first (permuted) column
+                    const float* zc = reinterpret_cast<const float*>(z[c & 1]);
+                    f32x2 sc[4];
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) {                              // 4 columns per W2 load
-                        const ulonglong2 w = *reinterpret_cast<const ulonglong2*>(W2s + hf * CP + c * 32 + g * 4);
-                        float h[4];
+                    for (int t = 0; t < 32; t += 2) {                           // eq. 2 on two pipes
+                        const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
+                        const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
+                        const int a4 = (t >> 1) & 3;
+                        sc[a4] = t < 8 ? pack2(h0, h1) : fadd2(sc[a4], pack2(h0, h1));
+                    }
+                    const float csum = hsum2(fadd2(fadd2(sc[0], sc[1]), fadd2(sc[2], sc[3])));
+                    yp = fmaf(cb < npos ? 1.f : -1.f, csum, yp);                // eq. 3: sign of the chunk
+                    if (cb < npos && npos < cb + 32) {                          // chunk with both signs
+                        f32x2 corr = 0ull;
 #pragma unroll
-                        for (int t = 0; t < 4; ++t) {
-                            const float zz = __uint_as_float(z[c & 1][g * 4 + t]);
-                            h[t] = g < 6 ? fmaxf(zz, 0.f) : zz + fabsf(zz);     // eq. 2 (ALU pipe / FMA pipe)
+                        for (int t = 0; t < 32; t += 2) {
+                            const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
+                            const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
+                            ffma2(corr, pack2(h0, h1), negmask[t >> 1]);
                         }
-                        ffma2(acc[(2 * g) & 3], pack2(h[0], h[1]), w.x);       // eq. 3
-                        ffma2(acc[(2 * g + 1) & 3], pack2(h[2], h[3]), w.y);
+                        yp = fmaf(-2.f, hsum2(corr), yp);
                     }
                     if (c + 1 < CP / 32) tmem_ld_wait();
                     if (c + 2 == CP / 32 || CP == 32) {
                         // every column of this part is now in registers: hand it back to the MMA warp
                         tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(bar_tempty + 8 * (2 * e + hf));
+                        if (lane == 0) mbar_arrive(bar_tempty + 8 * (NH * e + hf));
                     }
                 }
             }
-            const float yp = (hsum2(acc[0]) + hsum2(acc[1])) + (hsum2(acc[2]) + hsum2(acc[3]));
             const float err = row < n ? yp - yv : 0.f;
-            sse32 = fmaf(err, err, sse32);                                     // eq. 4
-            if (((i >> 1) & 31) == 31) { sse += (double)sse32; sse32 = 0.f; }  // fp64 every 32 tiles
+            const float t = fmaf(err, err, -comp);                             // eq. 4, Kahan-compensated fp32
+            const float su = sse32 + t;
+            comp = (su - sse32) - t;
+            sse32 = su;
         }
-        sse += (double)sse32;
+        sse = (double)sse32;
         for (int o = 16; o > 0; o >>= 1) sse += __shfl_down_sync(0xffffffffu, sse, o);
         if (lane == 0) wsum[warp - 2] = sse;
     }
@@ -275,7 +317,7 @@ cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const
                      double* partials, int grid, double* d_out, cudaStream_t stream) {
     auto kern = k_eval_tf32<H>;
     const size_t smem = (size_t)H * kIn * 4 + (size_t)kStages * kTileBytes + (size_t)H * 4 +
-                        8 * (2 * kStages + 8) + 8 * 8 + 16;
+                        8 * (2 * kStages + 16) + 8 * 8 + 4 * H + 32 + 4 + 16;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     unsigned int* ticket = reinterpret_cast<unsigned int*>(partials + grid);
