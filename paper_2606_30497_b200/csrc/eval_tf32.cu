@@ -99,11 +99,9 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     extern __shared__ __align__(1024) unsigned char smem[];
     float* Bs = reinterpret_cast<float*>(smem);                            // [H][32] swizzled
     unsigned char* Xring = smem + H * kIn * 4;                             // [kStages][16 KB]
-    float* W2s = reinterpret_cast<float*>(Xring + kStages * kTileBytes);   // [H]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(W2s + H);                 // full, empty, tfull[2][NH], tempty[2][NH]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Xring + kStages * kTileBytes);               // full, empty, tfull[2][NH], tempty[2][NH]
     double* wsum = reinterpret_cast<double*>(bars + 2 * kStages + 16);      // [8]
-    int* colmap = reinterpret_cast<int*>(wsum + 8);                        // [H] permuted column of unit j
-    int* wcnt = colmap + H;                                                // [8]
+    int* wcnt = reinterpret_cast<int*>(wsum + 8);                          // [8]
     int* npos_s = wcnt + 8;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(npos_s + 1);
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kStages),
@@ -121,25 +119,31 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     // of every chunk take ReLU as (z + |z|) on the FMA pipe and carry a factor 1/2.
     {
         const bool mine = tid < H;
-        const float w2v = mine ? W2[tid] : -1.f;
+        // thread j0 < H stages column j0 of W1: 32 independent coalesced loads in flight at once
+        float wcol[kIn];
+#pragma unroll
+        for (int k = 0; k < kIn; ++k) wcol[k] = mine ? __ldg(W1 + (size_t)k * H + tid) : 0.f;
+        const float w2v = mine ? __ldg(W2 + tid) : -1.f;
         const unsigned bal = __ballot_sync(0xffffffffu, mine && w2v >= 0.f);
         if (mine && lane == 0) wcnt[warp] = __popc(bal);
         __syncthreads();
         if (mine) {
             int before = __popc(bal & ((1u << lane) - 1u)), total = 0;
             for (int w = 0; w < H / 32; ++w) { const int c = wcnt[w]; total += c; if (w < warp) before += c; }
-            const int dest = w2v >= 0.f ? before : total + (tid - before);
-            colmap[tid] = dest;
-            W2s[tid] = ((dest & 31) >= 24 ? 0.5f : 1.0f) * fabsf(w2v);
+            // chunk 0 takes the first r0 units with w2 >= 0 and the first 32 - r0 with w2 < 0, the
+            // other (npos - r0, a multiple of 32) non-negative ones follow, then the negative ones
+            const int r0 = (total & 31) ? (total & 31) : (total > 0 ? 32 : 0);
+            const int a = before, b = tid - before;                         // rank among its sign
+            const int j = w2v >= 0.f ? (a < r0 ? a : 32 + (a - r0))
+                                     : (b < 32 - r0 ? r0 + b : total + b);  // permuted column = B row
+            const float sc = ((j & 31) >= 24 ? 0.5f : 1.0f) * fabsf(w2v);
             if (tid == 0) *npos_s = total;
+            unsigned char* brow = smem + (j >> 3) * 1024 + (j & 7) * 128;    // K-major row, 128B swizzle
+#pragma unroll
+            for (int c = 0; c < kIn / 4; ++c)
+                *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
+                    make_float4(wcol[4 * c] * sc, wcol[4 * c + 1] * sc, wcol[4 * c + 2] * sc, wcol[4 * c + 3] * sc);
         }
-        __syncthreads();
-    }
-    for (int idx = tid; idx < H * kIn; idx += kEvalThreads) {
-        const int j0 = idx % H, k = idx / H;                                // coalesced over j0
-        const int j = colmap[j0];                                           // permuted column = B row
-        const int off = (j >> 3) * 1024 + (j & 7) * 128 + ((((k >> 2) ^ (j & 7)) << 4) | ((k & 3) << 2));
-        *reinterpret_cast<float*>(smem + off) = W1[(size_t)k * H + j0] * W2s[j0];
     }
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
@@ -209,10 +213,10 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
         // ===== epilogue: set e handles tiles i with (i & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
         const int e = (warp - 2) >> 2, q = warp & 3;
         float sse32 = 0.f, comp = 0.f;
-        f32x2 negmask[16];                               // 1 for the w2 < 0 columns of the mixed chunk
+        const int r0 = (npos & 31) ? (npos & 31) : (npos > 0 ? 32 : 0);   // non-negative units in chunk 0
+        f32x2 sgn0[16];                                                  // +-1 weights of chunk 0
 #pragma unroll
-        for (int t = 0; t < 16; ++t)
-            negmask[t] = pack2((2 * t) >= (npos & 31) ? 1.f : 0.f, (2 * t + 1) >= (npos & 31) ? 1.f : 0.f);
+        for (int t = 0; t < 16; ++t) sgn0[t] = pack2(2 * t < r0 ? 1.f : -1.f, 2 * t + 1 < r0 ? 1.f : -1.f);
         for (uint32_t i = e; i < nt; i += 2) {
             const long long row = (blockIdx.x + (long long)i * gridDim.x) * kTile + q * 32 + lane;
             const float yv = row < n ? __ldg(Y + row) : 0.f;
@@ -236,20 +240,16 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
                         const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
                         const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
                         const int a4 = (t >> 1) & 3;
-                        sc[a4] = t < 8 ? pack2(h0, h1) : fadd2(sc[a4], pack2(h0, h1));
+                        if (hf == 0 && c == 0) {                                // chunk 0: signed sum
+                            if (t < 8) sc[a4] = fmul2(pack2(h0, h1), sgn0[t >> 1]);
+                            else ffma2(sc[a4], pack2(h0, h1), sgn0[t >> 1]);
+                        } else {
+                            sc[a4] = t < 8 ? pack2(h0, h1) : fadd2(sc[a4], pack2(h0, h1));
+                        }
                     }
                     const float csum = hsum2(fadd2(fadd2(sc[0], sc[1]), fadd2(sc[2], sc[3])));
-                    yp = fmaf(cb < npos ? 1.f : -1.f, csum, yp);                // eq. 3: sign of the chunk
-                    if (cb < npos && npos < cb + 32) {                          // chunk with both signs
-                        f32x2 corr = 0ull;
-#pragma unroll
-                        for (int t = 0; t < 32; t += 2) {
-                            const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
-                            const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
-                            ffma2(corr, pack2(h0, h1), negmask[t >> 1]);
-                        }
-                        yp = fmaf(-2.f, hsum2(corr), yp);
-                    }
+                    if (hf == 0 && c == 0) yp += csum;                           // signs applied per column
+                    else yp = fmaf(cb - 32 < npos - r0 ? 1.f : -1.f, csum, yp);  // eq. 3: sign of the chunk
                     if (c + 1 < CP / 32) tmem_ld_wait();
                     if (c + 2 == CP / 32 || CP == 32) {
                         // every column of this part is now in registers: hand it back to the MMA warp

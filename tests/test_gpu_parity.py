@@ -222,6 +222,22 @@ def test_eval_tf32_variant(hidden, n):
     assert gpu_eval(X, Y, W1, W2, variant=B.VARIANT_TF32) == lg      # deterministic
 
 
+@pytest.mark.parametrize("hidden", [32, 64, 256])
+@pytest.mark.parametrize("npos", ["all", "none", 1, 31, 32, 33, 64])
+def test_eval_tf32_sign_layouts(hidden, npos):
+    """The TF32 kernel sorts hidden units by the sign of W2: cover every boundary position."""
+    n = 3000
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(7, 32, hidden)
+    W2 = np.abs(W2) + np.float32(1e-3)
+    k = hidden if npos == "all" else 0 if npos == "none" else min(int(npos), hidden)
+    rng = np.random.default_rng(11)
+    neg = rng.permutation(hidden)[k:]
+    W2[neg] = -W2[neg]
+    lg, lo = gpu_eval(X, Y, W1, W2, variant=B.VARIANT_TF32), O.eval_loss(X, Y, W1, W2)
+    assert abs(lg - lo) <= 5e-3 * lo, (hidden, npos, lg, lo)
+
+
 def test_eval_tf32_unsupported_hidden():
     X, Y = datagen.make_dataset(256, 0.1)
     W1, W2 = O.init_weights(5, 32, 512)
