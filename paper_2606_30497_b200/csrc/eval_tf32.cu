@@ -28,7 +28,7 @@ namespace {
 
 constexpr int kTile = 128;           // rows per MMA (M)
 constexpr int kStages = 6;           // X ring depth (6 x 16 KB)
-constexpr int kEvalThreads = 320;    // producer + MMA + 8 epilogue warps
+constexpr int kEvalThreads = 352;    // producer + MMA (even tiles) + 8 epilogue warps + MMA (odd tiles)
 constexpr uint32_t kTileBytes = kTile * kIn * 4;
 
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1,
@@ -181,16 +181,20 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
             __syncwarp();
             if (++st == kStages) { st = 0; eph ^= 1u; }
         }
-    } else if (warp == 1) {
-        // ===== MMA issuer (whole warp runs the loop, one elected lane issues) =====
+    } else if (warp == 1 || warp == 10) {
+        // ===== MMA issuers: warp 1 feeds accumulator 0 (even tiles), warp 10 accumulator 1 (odd tiles), so
+        // that neither epilogue set ever waits behind the other set's TMEM hand-back (whole warp runs
+        // the loop, one elected lane issues) =====
         // instruction descriptor: D=f32, A=B=tf32, both K-major, N=CP, M=128
         constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(CP >> 3) << 17) |
                                    ((uint32_t)(kTile >> 4) << 24);
+        static_assert(kStages % 2 == 0, "a tile parity keeps to its ring stages");
         const uint64_t bdesc = smem_desc_sw128(smem_u32(Bs));
         const uint64_t adesc0 = smem_desc_sw128(smem_u32(Xring));
-        uint32_t st = 0, fph = 0;
-        for (uint32_t i = 0; i < nt; ++i) {
-            const uint32_t b = i & 1u, tph = ((i >> 1) - 1u) & 1u;
+        const uint32_t b = warp == 1 ? 0u : 1u;
+        uint32_t st = b, fph = 0;
+        for (uint32_t i = b; i < nt; i += 2) {
+            const uint32_t tph = ((i >> 1) - 1u) & 1u;
             mbar_wait(bar_full + 8 * st, fph);
             const uint64_t adesc = adesc0 + (uint64_t)(st * (kTileBytes >> 4));
 #pragma unroll
@@ -207,7 +211,8 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
                 }
                 __syncwarp();
             }
-            if (++st == kStages) { st = 0; fph ^= 1u; }
+            st += 2;
+            if (st >= kStages) { st -= kStages; fph ^= 1u; }
         }
     } else {
         // ===== epilogue: set e handles tiles i with (i & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
