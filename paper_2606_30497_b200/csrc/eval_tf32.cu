@@ -9,9 +9,11 @@
 // Persistent grid, one CTA per SM, warp-specialised:
 //   warp 0      TMA producer: 128-row X tiles (16 KB) by cp.async.bulk.tensor with the 128-byte
 //               swizzle the MMA wants, into a kStages-deep ring;
-//   warp 1      MMA issuer: per tile and column part four tcgen05.mma (M=128, N=hidden/NH, K=8)
-//               into one of two TMEM accumulators (2 x 256 columns = all of TMEM);
-//               tcgen05.commit releases the ring slot and publishes the accumulator part;
+//   warp 1, 10  MMA issuers (even / odd tiles): per tile and column part four tcgen05.mma
+//               (M=128, N=hidden/NH, K=8) into the TMEM accumulator of that tile parity
+//               (2 x 256 columns = all of TMEM); tcgen05.commit releases the ring slot and
+//               publishes the accumulator part.  One issuer per accumulator, so an epilogue set
+//               never waits behind the other set's hand-back;
 //   warps 2-9   epilogue, two sets of four warps (even / odd tiles, one TMEM accumulator each):
 //               a thread owns one row, streams its hidden row out of TMEM (tcgen05.ld 32x32b),
 //               applies eqs. 2-3 (ReLU + signed sum: |W2| is folded into the B operand, see
@@ -113,10 +115,10 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     // W2 is folded into the B operand: column j of Z' = X (W1 diag|W2|) is |w2_j| z_j, and
     //   w2_j ReLU(z_j) = sign(w2_j) ReLU(z'_j),
     // so the epilogue needs no multiply and no W2 operand (the W2 loads used to take as many
-    // shared-memory cycles as the MMA operand reads).  Hidden units are permuted so that the
-    // npos units with w2 >= 0 come first: a 32-column chunk then has one sign, except the chunk
-    // holding column npos, which is corrected with 0/1 masks kept in registers.  Columns 24..31
-    // of every chunk take ReLU as (z + |z|) on the FMA pipe and carry a factor 1/2.
+    // shared-memory cycles as the MMA operand reads).  Hidden units are permuted so that every
+    // 32-column chunk has one sign, except chunk 0, which collects the remainder of both signs and
+    // is summed with +-1 weights kept in registers.  Columns 24..31 of every chunk take ReLU as
+    // (z + |z|) on the FMA pipe and carry a factor 1/2.
     {
         const bool mine = tid < H;
         // thread j0 < H stages column j0 of W1: 32 independent coalesced loads in flight at once
