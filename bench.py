@@ -152,7 +152,7 @@ def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
     from paper_2606_30497_b200 import binding as B
-    from paper_2606_30497_b200 import datagen, roofline
+    from paper_2606_30497_b200 import datagen, roofline, sharding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference "
@@ -208,9 +208,7 @@ def run_ours(args, rank, world, local_rank):
     stats = B.mlp_get_train_stats()
     final_loss = float(dloss.item())
     if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+        total_ms = sharding.max_over_ranks(total_ms)      # device time of the slowest replica
     if rank != 0:
         return
 
