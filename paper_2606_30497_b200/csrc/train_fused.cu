@@ -214,32 +214,58 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             for (int u = 0; u < 4; ++u) w2r[u] = W2s[lu + u * LPS];
             {
                 // ---------------- forward: eqs. 1-3 (W1 columns in registers) ----------------
+                // The 32 LDS.128 that bring a lane's four W1 columns back cost 4 shared-memory cycles
+                // each (no broadcast across quarter-warps), ~1,000 cycles per CTA: the first row group
+                // is therefore processed chunk-major (4 inputs at a time) with the weight chunk loaded
+                // just ahead of its FFMA2s, so the reload overlaps the FMAs instead of preceding them.
                 f32x2 w[4][16];
-#pragma unroll
-                for (int q = 0; q < 8; ++q)
+                auto load_w_chunk = [&](int q) {
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const ulonglong2 a =
                             *reinterpret_cast<const ulonglong2*>(W1s + (q * S + lu + u * LPS) * 4);
                         w[u][2 * q] = a.x; w[u][2 * q + 1] = a.y;
                     }
+                };
                 mbar_wait(bar_full + 8 * xst, xph);
+                f32x2 z0[ITS][4];                       // Z1 accumulators of row group 0
+                load_w_chunk(0);
+#pragma unroll
+                for (int x = 0; x < 8; ++x) {
+                    if (x + 1 < 8) load_w_chunk(x + 1);
+                    asm volatile("" ::: "memory");      // keep the later chunks' loads behind these FMAs
+#pragma unroll
+                    for (int k = 0; k < ITS; ++k) {
+                        const ulonglong2 xv = reinterpret_cast<const ulonglong2*>(Xl + k * kIn)[x];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (x == 0) z0[k][u] = fmul2(xv.x, w[u][0]);                // eq. 1
+                            else ffma2(z0[k][u], xv.x, w[u][2 * x]);
+                            ffma2(z0[k][u], xv.y, w[u][2 * x + 1]);
+                        }
+                    }
+                }
 #pragma unroll
                 for (int q = 0; q < NSPLIT; ++q) {
                     float pv[ITS];
 #pragma unroll
                     for (int k = 0; k < ITS; ++k) {
                         const int it = q * ITS + k;
-                        const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xl + it * kIn);
-                        f32x2 a[4] = {0ull, 0ull, 0ull, 0ull};
+                        f32x2 a[4];
+                        if (q == 0) {
 #pragma unroll
-                        for (int x = 0; x < 8; ++x) {
-                            const ulonglong2 xv = xrow[x];
+                            for (int u = 0; u < 4; ++u) a[u] = z0[k][u];
+                        } else {
+                            const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xl + it * kIn);
 #pragma unroll
-                            for (int u = 0; u < 4; ++u) {
-                                if (x == 0) a[u] = fmul2(xv.x, w[u][0]);                // eq. 1
-                                else ffma2(a[u], xv.x, w[u][2 * x]);
-                                ffma2(a[u], xv.y, w[u][2 * x + 1]);
+                            for (int x = 0; x < 8; ++x) {
+                                const ulonglong2 xv = xrow[x];
+#pragma unroll
+                                for (int u = 0; u < 4; ++u) {
+                                    if (x == 0) a[u] = fmul2(xv.x, w[u][0]);            // eq. 1
+                                    else ffma2(a[u], xv.x, w[u][2 * x]);
+                                    ffma2(a[u], xv.y, w[u][2 * x + 1]);
+                                }
                             }
                         }
 #pragma unroll
