@@ -116,6 +116,7 @@ int check_train_args(const float* X, const float* Y, int64_t n, int batch, float
     if (((uintptr_t)Y & 3) || ((uintptr_t)W2 & 3))
         return fail(MLP_ERR_ALIGN, "Y and W2 must be 4-byte aligned");
     const int64_t nb = (n + batch - 1) / batch;
+    if (nb > 0x7fffffffLL) return fail(MLP_ERR_BAD_ARG, "too many batches per epoch (batch indices are int32)");
     if (nb * (int64_t)epochs > (int64_t)1 << 40) return fail(MLP_ERR_BAD_ARG, "too many steps");
     return MLP_OK;
 }

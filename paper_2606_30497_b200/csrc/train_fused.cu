@@ -49,6 +49,11 @@ struct TrainParams {
     const int* order;
     int H;
     unsigned long long* stats;
+    // host-precomputed bookkeeping (keeps 64-bit arithmetic and divisions out of the step loop)
+    int nbi;            // batches per epoch
+    int m_last;         // rows of the last batch of an epoch (== B when B divides n)
+    float scale_full;   // 2 / B       (eq. 5)
+    float scale_last;   // 2 / m_last
 };
 
 // Sum NV per-lane values across the L lanes of a sample group.  On return v[0] of the lane with
@@ -126,9 +131,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     cluster_sync_all();        // every CTA's barriers exist before anyone pushes to them
 
     const long long total = p.total_steps;
-    auto batch_index = [&](long long step) -> int {
-        return p.order ? __ldg(p.order + step) : (int)(step % p.nb);
-    };
+    // batch of a step: the order table, else sequential; `seq` counts steps modulo nb without division
+    int seq = 0;                                      // (step + 2) % nb for the look-ahead below
+    auto batch_index = [&](long long step, int sq) -> int { return p.order ? __ldg(p.order + step) : sq; };
+    auto rows_of = [&](int t) -> int { return t == p.nbi - 1 ? p.m_last : p.B; };
     // producer (one thread): bring `rows` rows starting at global row g0 into ring stage nbuf
     auto issue_tile = [&](long long g0, int rows, unsigned nbuf) {
         const uint32_t bar = bar_full + 8 * nbuf;
@@ -141,11 +147,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                          rb * 128, bar);
         }
     };
-    int t_cur = batch_index(0);
-    int t_next = total > 1 ? batch_index(1) : 0;
+    int t_cur = batch_index(0, 0);
+    int t_next = total > 1 ? batch_index(1, 1 % p.nbi) : 0;
+    seq = 2 % p.nbi;
     if (warp == 0 && lane == 0) {
         const long long r0 = (long long)t_cur * p.B;
-        const int m = (int)min((long long)p.B, p.n - r0);
+        const int m = rows_of(t_cur);
         issue_tile(r0, min(BT, m), 0);
     }
 
@@ -164,16 +171,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     float ycur = 0.f;
     {
         const long long r0 = (long long)t_cur * p.B;
-        const int m = (int)min((long long)p.B, p.n - r0);
+        const int m = rows_of(t_cur);
         if (yholder && yrow < min(BT, m)) ycur = __ldg(p.Y + r0 + yrow);
     }
     unsigned gt = 0;   // global tile counter
     for (long long step = 0; step < total; ++step) {
-        const int t_nn = (step + 2 < total) ? batch_index(step + 2) : 0;
+        const int t_nn = (step + 2 < total) ? batch_index(step + 2, seq) : 0;
+        seq = seq + 1 == p.nbi ? 0 : seq + 1;
         const long long r0 = (long long)t_cur * p.B;
-        const int m = (int)min((long long)p.B, p.n - r0);
+        const int m = rows_of(t_cur);
         const int ntiles = (m + BT - 1) / BT;
-        const float scale = 2.0f / (float)m;                  // eq. 5
+        const float scale = t_cur == p.nbi - 1 ? p.scale_last : p.scale_full;   // eq. 5: 2 / m
         float g2[4] = {0.f, 0.f, 0.f, 0.f};                   // dW2 partials (eq. 6)
 
         for (int j = 0; j < ntiles; ++j, ++gt) {
@@ -189,7 +197,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             if (j + 1 < ntiles) { nr0 = r0 + (long long)(j + 1) * BT; nrows = min(BT, m - (j + 1) * BT); }
             else if (step + 1 < total) {
                 nr0 = (long long)t_next * p.B;
-                nrows = (int)min((long long)min(BT, p.B), p.n - nr0);
+                nrows = min(BT, rows_of(t_next));
             }
             if (warp == 0 && lane == 0) {
                 // arm this tile's exchange barriers
@@ -535,6 +543,10 @@ cudaError_t launch_train_fused(const float* X, const float* Y, int64_t n, int ba
     p.X = X; p.Y = Y; p.n = n; p.B = batch; p.lr = lr;
     p.nb = (n + batch - 1) / batch;
     p.total_steps = (long long)epochs * p.nb;
+    p.nbi = (int)p.nb;
+    p.m_last = (int)(n - (p.nb - 1) * batch);
+    p.scale_full = 2.0f / (float)batch;
+    p.scale_last = 2.0f / (float)p.m_last;
     p.W1 = W1; p.W2 = W2; p.order = order; p.H = hidden; p.stats = stats;
     if (p.total_steps == 0) return cudaSuccess;
     cudaError_t err;
