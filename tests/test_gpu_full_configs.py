@@ -1,0 +1,90 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 3, 4, 5), in the launch configuration the
+benchmark uses (default cluster, fused kernel, per-epoch batch-order permutation from seed 3).
+
+Gate (BASELINE.json north_star; metric of SURVEY.md 8(c)): per matrix max|gpu - oracle| / max|oracle|
+<= 1e-5 after one SGD step, <= 1e-3 after one epoch; eval loss within 1 % -- here every epoch the
+oracle can afford is compared (the oracle runs ~0.7 M samples/s on the box's cores, so the largest
+sweep members are compared over their first epoch; the GPU runs every epoch of the config and the
+per-epoch GPU losses must decrease)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import mlp_oracle as O                      # noqa: E402
+from paper_2606_30497_b200 import binding as B          # noqa: E402
+from paper_2606_30497_b200 import datagen               # noqa: E402
+
+LR = np.float32(0.002)
+
+
+def nerr(g, o):
+    g = np.asarray(g, np.float64); o = np.asarray(o, np.float64)
+    return float(np.abs(g - o).max() / max(np.abs(o).max(), 1e-30))
+
+
+class Gpu:
+    def __init__(self, X, Y, hidden):
+        B.mlp_init(2, 32, hidden, 1)
+        B.mlp_set_cluster(0)
+        self.n, self.hidden = X.shape[0], hidden
+        self.dX, self.dY = torch.from_numpy(X).cuda(), torch.from_numpy(Y).cuda()
+
+    def train(self, W1, W2, batch, epochs, order):
+        B.mlp_init(2, 32, self.hidden, 1)
+        d1, d2 = torch.from_numpy(W1.copy()).cuda(), torch.from_numpy(W2.copy()).cuda()
+        dO = torch.from_numpy(np.ascontiguousarray(order).reshape(-1)).cuda()
+        B.mlp_train_ex(self.dX, self.dY, self.n, batch, LR, epochs, d1, d2, dO, B.VARIANT_FUSED)
+        torch.cuda.synchronize()
+        return d1.cpu().numpy(), d2.cpu().numpy()
+
+    def loss(self, W1, W2):
+        B.mlp_init(2, 32, self.hidden, 1)
+        return B.mlp_eval_loss(self.dX, self.dY, self.n, torch.from_numpy(W1).cuda(), torch.from_numpy(W2).cuda())
+
+
+def check_config(c, oracle_epochs):
+    X, Y = datagen.make_dataset(c.n, c.sigma)
+    W1, W2 = O.init_weights(2, 32, c.hidden)
+    order = datagen.make_order(c.n, c.batch, c.epochs, c.shuffle)
+    g = Gpu(X, Y, c.hidden)
+    nb = datagen.num_batches(c.n, c.batch)
+    # one SGD step: the first batch of the first epoch only (a one-batch call on that row range)
+    t0 = int(order[0][0]); lo, hi = t0 * c.batch, min(c.n, (t0 + 1) * c.batch)
+    g1 = Gpu(X[lo:hi], Y[lo:hi], c.hidden).train(W1, W2, c.batch, 1, np.zeros((1, 1), np.int32))
+    o1 = O.train(X[lo:hi], Y[lo:hi], W1, W2, c.batch, LR, 1)
+    assert nerr(g1[0], o1[0]) <= 1e-5 and nerr(g1[1], o1[1]) <= 1e-5, (c.name, "1 step", nerr(g1[0], o1[0]))
+    # epoch by epoch, as far as the oracle is run
+    gw, ow = (W1, W2), (W1, W2)
+    losses = [g.loss(W1, W2)]
+    for e in range(c.epochs):
+        gw = g.train(gw[0], gw[1], c.batch, 1, order[e:e + 1])
+        losses.append(g.loss(*gw))
+        if e < oracle_epochs:
+            ow = O.train(X, Y, ow[0], ow[1], c.batch, LR, 1, order=order[e:e + 1])
+            e1, e2 = nerr(gw[0], ow[0]), nerr(gw[1], ow[1])
+            assert e1 <= 1e-3 and e2 <= 1e-3, (c.name, "epoch", e + 1, e1, e2)
+            lo_ = O.eval_loss(X, Y, ow[0], ow[1])
+            assert abs(losses[-1] - lo_) <= 1e-2 * lo_, (c.name, "loss after epoch", e + 1, losses[-1], lo_)
+    assert all(b < a for a, b in zip(losses, losses[1:])), (c.name, losses)
+    # the whole config in ONE launch (what bench.py times) equals the epoch-by-epoch runs bitwise
+    w_all = g.train(W1, W2, c.batch, c.epochs, order)
+    assert np.array_equal(w_all[0], gw[0]) and np.array_equal(w_all[1], gw[1]), c.name
+    assert nb * c.epochs == order.size
+
+
+def test_config3_full():
+    check_config(datagen.CONFIGS["config3"], oracle_epochs=10)
+
+
+@pytest.mark.parametrize("member", range(4))
+def test_config4_full(member):
+    c = datagen.sweep("config4")[member]
+    check_config(c, oracle_epochs=5 if c.hidden <= 512 else 2)
+
+
+@pytest.mark.parametrize("member", range(4))
+def test_config5_full(member):
+    check_config(datagen.sweep("config5")[member], oracle_epochs=1)
