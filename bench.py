@@ -322,6 +322,39 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     unfused_us = a.elapsed_time(b) * 1e3 / datagen.num_batches(cfg.n, cfg.batch)
 
+    # ---- the paper's own shapes (Tables I-II): seconds for 100 epochs, B=256, sequential
+    #      batches, with the paper's two strategies re-created (prior_art.cu) beside the fused kernel ----
+    paper_T4 = {"n256": (0.306, 0.248), "n2560": (2.000, 1.561), "n25600": (21.002, 14.823),
+                "h32": 0.810, "h64": 0.921, "h128": 1.107, "h256": 1.551, "h512": 2.743, "h1024": 4.645}
+
+    def seconds(nn, hidden, variant, epochs=100):
+        B.mlp_init(2, 32, hidden, 1)
+        a1 = torch.empty(32, hidden, device="cuda"); a2 = torch.empty(hidden, device="cuda")
+        B.mlp_init_weights(a1, a2)
+        ep = epochs if variant == B.VARIANT_FUSED else max(1, min(epochs, 2000 // max(1, nn // 256)))
+        B.mlp_train_ex(dXp, dYp, nn, 256, cfg.lr, 1, a1, a2, None, variant)          # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        B.mlp_train_ex(dXp, dYp, nn, 256, cfg.lr, ep, a1, a2, None, variant)
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) * epochs / ep
+
+    Xp, Yp = datagen.make_dataset(25600, cfg.sigma)
+    dXp, dYp = torch.from_numpy(Xp).cuda(), torch.from_numpy(Yp).cuda()
+    paper_shapes = {"unit": "seconds per 100 epochs (host wall clock incl. launches; baselines extrapolated "
+                            "from >= 2000 SGD steps)", "table1": {}, "table2_n2560": {}}
+    for nn in (256, 2560, 25600):
+        naive, tiled, fused = (seconds(nn, 256, v) for v in (B.VARIANT_PRIOR_NAIVE, B.VARIANT_PRIOR_TILED, B.VARIANT_FUSED))
+        paper_shapes["table1"]["n%d" % nn] = {
+            "paper_T4_baseline": paper_T4["n%d" % nn][0], "paper_T4_optimized": paper_T4["n%d" % nn][1],
+            "b200_paper_baseline": naive, "b200_paper_optimized": tiled, "b200_fused": fused,
+            "b200_optimized_over_baseline": naive / tiled}
+    for hh in (32, 64, 128, 256, 512, 1024):
+        paper_shapes["table2_n2560"]["h%d" % hh] = {
+            "paper_T4": paper_T4["h%d" % hh], "b200_paper_optimized": seconds(2560, hh, B.VARIANT_PRIOR_TILED),
+            "b200_fused": seconds(2560, hh, B.VARIANT_FUSED)}
+    B.mlp_init(2, 32, cfg.hidden, 1)
+
     cpu = oracle_leg(cfg, X, Y, W1i.cpu().numpy(), W2i.cpu().numpy(), order)
 
     line = {
@@ -337,7 +370,7 @@ def run_ours(args, rank, world, local_rank):
         "us_per_sgd_step": us_per_sgd, "final_loss": final_loss,
         "roofline": roof, "train_by_cluster": by_cluster, "eval_4M_rows": best, "e2e": e2e, "e2e_bitwise_equal_to_device_path": e2e_matches,
         "gpu_launches": int(launches), "unfused_baseline_us_per_sgd_step": unfused_us,
-        "cpu_baseline": cpu, "clocks": sampler.summary(),
+        "paper_shapes": paper_shapes, "cpu_baseline": cpu, "clocks": sampler.summary(),
         "context": "paper (Tesla T4, optimised kernels): 1,482 us/step, 172.7 k samples/s (PAPER.md:330, derived)",
     }
     print(json.dumps(line))

@@ -18,6 +18,8 @@ MLP_OK = 0
 VARIANT_FUSED = 0
 VARIANT_UNFUSED = 1
 VARIANT_TF32 = 2
+VARIANT_PRIOR_NAIVE = 3
+VARIANT_PRIOR_TILED = 4
 
 EXPORTS = [
     "mlp_init", "mlp_init_weights", "mlp_train", "mlp_train_ex", "mlp_eval_loss",

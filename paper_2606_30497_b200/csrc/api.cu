@@ -26,6 +26,7 @@ struct State {
     double* eval_out = nullptr;       // device double for the synchronous entry
     unsigned long long* stats = nullptr;
     UnfusedScratch unf = {};          int unf_batch = 0, unf_hidden = 0;
+    float *priorXT = nullptr, *priorHT = nullptr;   // transposes of the paper's tiled strategy
     float *hX = nullptr, *hY = nullptr, *hW1 = nullptr, *hW2 = nullptr; int32_t* hOrder = nullptr;
     size_t hX_cap = 0, hY_cap = 0, hW_cap = 0, hOrder_cap = 0;
     cudaStream_t host_stream = nullptr;
@@ -83,7 +84,8 @@ int ensure_eval_scratch(int grid) {
 
 int ensure_unfused(int batch, int hidden) {
     if (g.unf.Z1 && g.unf_batch >= batch && g.unf_hidden == hidden) return MLP_OK;
-    float** ptrs[] = {&g.unf.Z1, &g.unf.Hact, &g.unf.dZ1, &g.unf.Ypred, &g.unf.dZ2, &g.unf.dW1, &g.unf.dW2};
+    float** ptrs[] = {&g.unf.Z1, &g.unf.Hact, &g.unf.dZ1, &g.unf.Ypred, &g.unf.dZ2, &g.unf.dW1, &g.unf.dW2,
+                      &g.priorXT, &g.priorHT};
     for (auto pp : ptrs) if (*pp) { CK(cudaFree(*pp)); *pp = nullptr; }
     const size_t bh = (size_t)batch * hidden;
     CK(cudaMalloc(reinterpret_cast<void**>(&g.unf.Z1), bh * 4));
@@ -93,6 +95,8 @@ int ensure_unfused(int batch, int hidden) {
     CK(cudaMalloc(reinterpret_cast<void**>(&g.unf.dZ2), (size_t)batch * 4));
     CK(cudaMalloc(reinterpret_cast<void**>(&g.unf.dW1), (size_t)kIn * hidden * 4));
     CK(cudaMalloc(reinterpret_cast<void**>(&g.unf.dW2), (size_t)hidden * 4));
+    CK(cudaMalloc(reinterpret_cast<void**>(&g.priorXT), (size_t)batch * kIn * 4));
+    CK(cudaMalloc(reinterpret_cast<void**>(&g.priorHT), bh * 4));
     g.unf_batch = batch; g.unf_hidden = hidden;
     return MLP_OK;
 }
@@ -109,7 +113,8 @@ int check_train_args(const float* X, const float* Y, int64_t n, int batch, float
     if (batch < 1) return fail(MLP_ERR_BAD_ARG, "batch must be >= 1 (got %d)", batch);
     if (epochs < 0) return fail(MLP_ERR_BAD_ARG, "epochs must be >= 0 (got %d)", epochs);
     if (!std::isfinite(lr)) return fail(MLP_ERR_BAD_ARG, "lr must be finite");
-    if (variant != MLP_VARIANT_FUSED && variant != MLP_VARIANT_UNFUSED)
+    if (variant != MLP_VARIANT_FUSED && variant != MLP_VARIANT_UNFUSED &&
+        variant != MLP_VARIANT_PRIOR_NAIVE && variant != MLP_VARIANT_PRIOR_TILED)
         return fail(MLP_ERR_UNSUPPORTED, "training variant %d is not supported", variant);
     if (((uintptr_t)X & 15) || ((uintptr_t)W1 & 15))
         return fail(MLP_ERR_ALIGN, "X and W1 must be 16-byte aligned");
@@ -151,10 +156,15 @@ int train_impl(const float* X, const float* Y, int64_t n, int batch, float lr, i
         for (int32_t t : oh)
             if (t < 0 || t >= nb) return fail(MLP_ERR_BAD_ARG, "batch_order entry %d outside [0,%lld)", t, (long long)nb);
     }
-    cudaError_t e = launch_train_unfused(X, Y, n, batch, lr, epochs, W1, W2,
-                                         order ? oh.data() : nullptr, g.hidden, g.unf, stream,
-                                         &g.launches);
-    if (e != cudaSuccess) return cuda_fail(e, "launch_train_unfused");
+    cudaError_t e;
+    if (variant == MLP_VARIANT_UNFUSED)
+        e = launch_train_unfused(X, Y, n, batch, lr, epochs, W1, W2, order ? oh.data() : nullptr,
+                                 g.hidden, g.unf, stream, &g.launches);
+    else
+        e = launch_train_prior(variant == MLP_VARIANT_PRIOR_TILED, X, Y, n, batch, lr, epochs, W1, W2,
+                               order ? oh.data() : nullptr, g.hidden, g.unf, g.priorXT, g.priorHT,
+                               stream, &g.launches);
+    if (e != cudaSuccess) return cuda_fail(e, "launch_train_unfused/prior");
     return MLP_OK;
 }
 
@@ -345,7 +355,7 @@ const char* mlp_version(void) { return "libmlp_b200 0.1 (sm_100a)"; }
 void mlp_shutdown(void) {
     std::lock_guard<std::mutex> lk(g_mu);
     void* ptrs[] = {g.eval_partials, g.eval_out, g.stats, g.unf.Z1, g.unf.Hact, g.unf.dZ1,
-                    g.unf.Ypred, g.unf.dZ2, g.unf.dW1, g.unf.dW2, g.hX, g.hY, g.hW1, g.hOrder};
+                    g.unf.Ypred, g.unf.dZ2, g.unf.dW1, g.unf.dW2, g.priorXT, g.priorHT, g.hX, g.hY, g.hW1, g.hOrder};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (g.host_stream) cudaStreamDestroy(g.host_stream);
     const bool init = g.init; const uint64_t seed = g.seed;

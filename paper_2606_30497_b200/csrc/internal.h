@@ -28,6 +28,11 @@ cudaError_t launch_train_unfused(const float* X, const float* Y, int64_t n, int 
                                  int epochs, float* W1, float* W2, const int32_t* order_host,
                                  int hidden, const UnfusedScratch& s, cudaStream_t stream,
                                  int64_t* launches);
+// prior_art.cu -- the paper's naive / tiled+transposed+fused strategies (comparison only, NEXT-4)
+cudaError_t launch_train_prior(bool tiled, const float* X, const float* Y, int64_t n, int batch, float lr,
+                               int epochs, float* W1, float* W2, const int32_t* order_host, int hidden,
+                               const UnfusedScratch& s, float* XT, float* HT, cudaStream_t stream,
+                               int64_t* launches);
 cudaError_t launch_init_weights(uint64_t seed, int hidden, float* W1, float* W2,
                                 cudaStream_t stream, int64_t* launches);
 

@@ -101,6 +101,18 @@ def test_config1_unfused_baseline(cfg1):
     assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5
 
 
+# The paper's own two strategies, re-created for comparison: same gates.
+@pytest.mark.parametrize("variant", ["PRIOR_NAIVE", "PRIOR_TILED"])
+@pytest.mark.parametrize("hidden,batch,n", [(256, 256, 2560), (64, 100, 1001), (1024, 256, 1000)])
+def test_paper_strategies_match_oracle(variant, hidden, batch, n):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(2, 32, hidden)
+    order = datagen.make_order(n, batch, 2, True)
+    o1, o2 = O.train(X, Y, W1, W2, batch, LR, 2, order=order)
+    g1, g2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=getattr(B, "VARIANT_" + variant))
+    assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5, (variant, nerr(g1, o1), nerr(g2, o2))
+
+
 # ------------------------------------------------------------------ config 2 (shuffled batch order)
 def test_config2_epoch_and_final_loss():
     c = datagen.CONFIGS["config2"]
