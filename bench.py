@@ -322,6 +322,27 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     unfused_us = a.elapsed_time(b) * 1e3 / datagen.num_batches(cfg.n, cfg.batch)
 
+    # ---- concurrent replicas: R independent models of the same job on R streams,
+    #      each a cluster of `cluster` SMs; aggregate samples/s over all models ----
+    conc = {}
+    for R in (4, 16):
+        streams = [torch.cuda.Stream() for _ in range(R)]
+        ws = [(W1i.clone(), W2i.clone()) for _ in range(R)]
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for st, (r1, r2) in zip(streams, ws):
+            st.wait_event(a)
+            with torch.cuda.stream(st):
+                B.mlp_train_ex(dX, dY, cfg.n, cfg.batch, cfg.lr, cfg.epochs, r1, r2, dO, B.VARIANT_FUSED)
+        for st in streams:
+            torch.cuda.current_stream().wait_stream(st)
+        b.record()
+        torch.cuda.synchronize()
+        same = all(torch.equal(r1, ws[0][0]) and torch.equal(r2, ws[0][1]) for r1, r2 in ws)
+        conc[str(R)] = {"ms": a.elapsed_time(b), "aggregate_samples_per_s": R * samples_per_step / (a.elapsed_time(b) * 1e-3),
+                        "replicas_bitwise_equal": bool(same)}
+
     # ---- the paper's own shapes (Tables I-II): seconds for 100 epochs, B=256, sequential
     #      batches, with the paper's two strategies re-created (prior_art.cu) beside the fused kernel ----
     paper_T4 = {"n256": (0.306, 0.248), "n2560": (2.000, 1.561), "n25600": (21.002, 14.823),
@@ -370,7 +391,7 @@ def run_ours(args, rank, world, local_rank):
         "us_per_sgd_step": us_per_sgd, "final_loss": final_loss,
         "roofline": roof, "train_by_cluster": by_cluster, "eval_4M_rows": best, "e2e": e2e, "e2e_bitwise_equal_to_device_path": e2e_matches,
         "gpu_launches": int(launches), "unfused_baseline_us_per_sgd_step": unfused_us,
-        "paper_shapes": paper_shapes, "cpu_baseline": cpu, "clocks": sampler.summary(),
+        "concurrent_replicas": conc, "paper_shapes": paper_shapes, "cpu_baseline": cpu, "clocks": sampler.summary(),
         "context": "paper (Tesla T4, optimised kernels): 1,482 us/step, 172.7 k samples/s (PAPER.md:330, derived)",
     }
     print(json.dumps(line))
