@@ -107,8 +107,7 @@ double mlp_eval_loss(const float* X, const float* Y, int64_t n,
  *   variant: MLP_VARIANT_FUSED = the exact-fp32 kernel of mlp_eval_loss (bound by the FP32 pipes);
  *            MLP_VARIANT_TF32  = eq. 1 on the tensor cores (tcgen05.mma kind::tf32: fp32 operands
  *            truncated to TF32, fp32 accumulate), the HBM-bound variant; stated tolerance: loss within
- *            1 % of the exact value (measured <= 1e-4 relative); hidden <= 256 and n < 2^31 - 128,
- *            otherwise MLP_ERR_UNSUPPORTED / MLP_ERR_CUDA.  X must be 16-byte aligned.  Deterministic. */
+ *            1 % of the exact value (measured <= 1e-4 relative); n < 2^31 - 128, otherwise MLP_ERR_CUDA.  X must be 16-byte aligned.  Deterministic. */
 int mlp_eval_loss_async(const float* X, const float* Y, int64_t n, const float* W1,
                         const float* W2, double* d_out, int variant, void* stream);
 

@@ -20,6 +20,7 @@
 //               "setup"), eq. 4 in compensated fp32 per thread, fp64 from the warp level up.
 //               Deterministic: fixed-order block and last-block reductions.
 // W1 diag|W2| is transposed once per CTA into the K-major swizzled B operand ([hidden][32] floats).
+// hidden > 256: 256-column slices of the same X tile alternate between the two accumulators.
 #include <cuda.h>
 
 #include "common.cuh"
@@ -86,30 +87,41 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
 
+// Hidden widths above 256 (one MMA N-extent, half of TMEM) are processed as NS = H/256 column
+// slices per tile: the X tile is read from HBM once, slice sl of a tile goes to accumulator
+// (sl & 1), and the two epilogue sets combine their per-row partial sums through shared memory.
+constexpr int eval_stages(int H) { return H >= 1024 ? 4 : kStages; }
+
 template <int H>
 __global__ void __launch_bounds__(kEvalThreads, 1)
 k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y, long long n,
             const float* __restrict__ W1, const float* __restrict__ W2,
             double* __restrict__ partials, unsigned int* __restrict__ ticket,
             double* __restrict__ out) {
-    static_assert(H % 32 == 0 && H >= 32 && H <= 256, "one MMA N-extent, 32-column TMEM loads");
+    static_assert(H % 32 == 0 && H >= 32 && H <= 1024 && (H <= 256 || H % 256 == 0), "hidden width");
+    constexpr int HS = H < 256 ? H : 256;      // columns per slice (one MMA N-extent at most)
+    constexpr int NS = H / HS;                 // slices per tile (1, 2 or 4)
     // Each 256-column TMEM accumulator is filled and drained in NH column parts, so the MMA of the
-    // next tile's first part overlaps the epilogue of this tile's second part.
-    constexpr int NH = H >= 128 ? 2 : 1;
-    constexpr int CP = H / NH;                 // columns (hidden units) per part
+    // next item's first part overlaps the epilogue of this item's second part.
+    constexpr int NH = HS >= 128 ? 2 : 1;
+    constexpr int CP = HS / NH;                // columns (hidden units) per part
+    constexpr int NST = eval_stages(H);        // X ring depth
+    constexpr int NG = H / 32;                 // 32-unit groups
     // 1024-byte alignment: swizzle atoms of both operands (checked below)
     extern __shared__ __align__(1024) unsigned char smem[];
     float* Bs = reinterpret_cast<float*>(smem);                            // [H][32] swizzled
-    unsigned char* Xring = smem + H * kIn * 4;                             // [kStages][16 KB]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(Xring + kStages * kTileBytes);               // full, empty, tfull[2][NH], tempty[2][NH]
-    double* wsum = reinterpret_cast<double*>(bars + 2 * kStages + 16);      // [8]
-    int* wcnt = reinterpret_cast<int*>(wsum + 8);                          // [8]
-    int* npos_s = wcnt + 8;
+    unsigned char* Xring = smem + H * kIn * 4;                             // [NST][16 KB]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Xring + NST * kTileBytes);   // full, empty, tfull[2][NH], tempty[2][NH]
+    double* wsum = reinterpret_cast<double*>(bars + 2 * NST + 16);         // [8]
+    float* rowpart = reinterpret_cast<float*>(wsum + 8);                   // [2][128] partial rows of set 1
+    int* wcnt = reinterpret_cast<int*>(rowpart + 2 * kTile);               // [32]
+    int* npos_s = wcnt + 32;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(npos_s + 1);
-    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kStages),
-                   bar_tfull = smem_u32(bars + 2 * kStages), bar_tempty = smem_u32(bars + 2 * kStages + 8);
+    const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + NST),
+                   bar_tfull = smem_u32(bars + 2 * NST), bar_tempty = smem_u32(bars + 2 * NST + 8);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    constexpr int NW = kEvalThreads / 32;
 
     // ---- setup -------------------------------------------------------------------------------------
     // W2 is folded into the B operand: column j of Z' = X (W1 diag|W2|) is |w2_j| z_j, and
@@ -119,36 +131,37 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     // 32-column chunk has one sign, except chunk 0, which collects the remainder of both signs and
     // is summed with +-1 weights kept in registers.  Columns 24..31 of every chunk take ReLU as
     // (z + |z|) on the FMA pipe and carry a factor 1/2.
-    {
-        const bool mine = tid < H;
-        // thread j0 < H stages column j0 of W1: 32 independent coalesced loads in flight at once
+    for (int g = warp; g < NG; g += NW) {                      // a warp per group of 32 hidden units
+        const unsigned bal = __ballot_sync(0xffffffffu, __ldg(W2 + g * 32 + lane) >= 0.f);
+        if (lane == 0) wcnt[g] = __popc(bal);
+    }
+    __syncthreads();
+    for (int g = warp; g < NG; g += NW) {
+        const int j0 = g * 32 + lane;
+        // lane stages column j0 of W1: 32 independent coalesced loads in flight at once
         float wcol[kIn];
 #pragma unroll
-        for (int k = 0; k < kIn; ++k) wcol[k] = mine ? __ldg(W1 + (size_t)k * H + tid) : 0.f;
-        const float w2v = mine ? __ldg(W2 + tid) : -1.f;
-        const unsigned bal = __ballot_sync(0xffffffffu, mine && w2v >= 0.f);
-        if (mine && lane == 0) wcnt[warp] = __popc(bal);
-        __syncthreads();
-        if (mine) {
-            int before = __popc(bal & ((1u << lane) - 1u)), total = 0;
-            for (int w = 0; w < H / 32; ++w) { const int c = wcnt[w]; total += c; if (w < warp) before += c; }
-            // chunk 0 takes the first r0 units with w2 >= 0 and the first 32 - r0 with w2 < 0, the
-            // other (npos - r0, a multiple of 32) non-negative ones follow, then the negative ones
-            const int r0 = (total & 31) ? (total & 31) : (total > 0 ? 32 : 0);
-            const int a = before, b = tid - before;                         // rank among its sign
-            const int j = w2v >= 0.f ? (a < r0 ? a : 32 + (a - r0))
-                                     : (b < 32 - r0 ? r0 + b : total + b);  // permuted column = B row
-            const float sc = ((j & 31) >= 24 ? 0.5f : 1.0f) * fabsf(w2v);
-            if (tid == 0) *npos_s = total;
-            unsigned char* brow = smem + (j >> 3) * 1024 + (j & 7) * 128;    // K-major row, 128B swizzle
+        for (int k = 0; k < kIn; ++k) wcol[k] = __ldg(W1 + (size_t)k * H + j0);
+        const float w2v = __ldg(W2 + j0);
+        const unsigned bal = __ballot_sync(0xffffffffu, w2v >= 0.f);
+        int before = __popc(bal & ((1u << lane) - 1u)), total = 0;
+        for (int w = 0; w < NG; ++w) { const int c = wcnt[w]; total += c; if (w < g) before += c; }
+        // chunk 0 takes the first r0 units with w2 >= 0 and the first 32 - r0 with w2 < 0, the
+        // other (npos - r0, a multiple of 32) non-negative ones follow, then the negative ones
+        const int r0 = (total & 31) ? (total & 31) : (total > 0 ? 32 : 0);
+        const int a = before, b = j0 - before;                          // rank among its sign
+        const int j = w2v >= 0.f ? (a < r0 ? a : 32 + (a - r0))
+                                 : (b < 32 - r0 ? r0 + b : total + b);  // permuted column = B row
+        const float sc = ((j & 31) >= 24 ? 0.5f : 1.0f) * fabsf(w2v);
+        if (j0 == 0) *npos_s = total;
+        unsigned char* brow = smem + (j >> 3) * 1024 + (j & 7) * 128;    // K-major row, 128B swizzle
 #pragma unroll
-            for (int c = 0; c < kIn / 4; ++c)
-                *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
-                    make_float4(wcol[4 * c] * sc, wcol[4 * c + 1] * sc, wcol[4 * c + 2] * sc, wcol[4 * c + 3] * sc);
-        }
+        for (int c = 0; c < kIn / 4; ++c)
+            *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
+                make_float4(wcol[4 * c] * sc, wcol[4 * c + 1] * sc, wcol[4 * c + 2] * sc, wcol[4 * c + 3] * sc);
     }
     if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+        for (int s = 0; s < NST; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NS > 1 ? 2 : 1); }
         for (int b = 0; b < 8; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
         fence_mbar_init();
     }
@@ -168,69 +181,74 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     const long long ntiles = (n + kTile - 1) / kTile;
     const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     double sse = 0.0;
-
     const uint32_t nt = (uint32_t)my_tiles;
+    // Work items: item w = i * NS + sl is slice sl of this CTA's i-th tile; it uses accumulator
+    // (w & 1), MMA issuer (w & 1) and epilogue set (w & 1).  nt * NS < 2^31 by the host check.
+    const uint32_t nitems = nt * NS;
+
     if (warp == 0) {
         // ===== TMA producer (whole warp runs the loop, one elected lane issues) =====
         uint32_t st = 0, eph = 1;                       // ring stage, parity of the "empty" phase to wait for
         for (uint32_t i = 0; i < nt; ++i) {
-            if (i >= kStages) mbar_wait(bar_empty + 8 * st, eph);
+            if (i >= NST) mbar_wait(bar_empty + 8 * st, eph);
             if (elect_one()) {
                 const long long row0 = (blockIdx.x + (long long)i * gridDim.x) * kTile;
                 mbar_arrive_expect_tx(bar_full + 8 * st, kTileBytes);   // OOB rows are zero-filled, still counted
                 tma_load_2d(smem_u32(Xring) + st * kTileBytes, &tmapX, 0, (int)row0, bar_full + 8 * st);
             }
             __syncwarp();
-            if (++st == kStages) { st = 0; eph ^= 1u; }
+            if (++st == NST) { st = 0; eph ^= 1u; }
         }
     } else if (warp == 1 || warp == 10) {
-        // ===== MMA issuers: warp 1 feeds accumulator 0 (even tiles), warp 10 accumulator 1 (odd tiles), so
+        // ===== MMA issuers: warp 1 feeds accumulator 0 (even items), warp 10 accumulator 1 (odd items), so
         // that neither epilogue set ever waits behind the other set's TMEM hand-back (whole warp runs
         // the loop, one elected lane issues) =====
         // instruction descriptor: D=f32, A=B=tf32, both K-major, N=CP, M=128
         constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(CP >> 3) << 17) |
                                    ((uint32_t)(kTile >> 4) << 24);
-        static_assert(kStages % 2 == 0, "a tile parity keeps to its ring stages");
         const uint64_t bdesc = smem_desc_sw128(smem_u32(Bs));
         const uint64_t adesc0 = smem_desc_sw128(smem_u32(Xring));
         const uint32_t b = warp == 1 ? 0u : 1u;
-        uint32_t st = b, fph = 0;
-        for (uint32_t i = b; i < nt; i += 2) {
-            const uint32_t tph = ((i >> 1) - 1u) & 1u;
-            mbar_wait(bar_full + 8 * st, fph);
+        for (uint32_t w = b, kth = 0; w < nitems; w += 2, ++kth) {
+            const uint32_t i = w / NS, sl = w % NS, st = i % NST;
+            const uint32_t tph = (kth - 1u) & 1u;
+            mbar_wait(bar_full + 8 * st, (i / NST) & 1u);
             const uint64_t adesc = adesc0 + (uint64_t)(st * (kTileBytes >> 4));
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) {
-                if (i >= 2) mbar_wait(bar_tempty + 8 * (NH * b + hf), tph);
+                if (kth >= 1) mbar_wait(bar_tempty + 8 * (NH * b + hf), tph);
                 tc_fence_after();
                 if (elect_one()) {
 #pragma unroll
                     for (int k = 0; k < kIn / 8; ++k)  // K = 8 tf32 = 32 bytes per MMA: +2 in 16-byte units
                         mma_tf32(tmem_base + b * 256 + hf * CP, adesc + 2 * k,
-                                 bdesc + (uint64_t)(hf * CP * 128 / 16) + 2 * k, idesc, k > 0);
-                    if (hf == NH - 1) tc_commit(bar_empty + 8 * st);   // ring slot free once read
+                                 bdesc + (uint64_t)((sl * HS + hf * CP) * 128 / 16) + 2 * k, idesc, k > 0);
+                    // ring slot free once the last slice this issuer takes from the tile has read it
+                    if (hf == NH - 1 && sl + 2 >= NS) tc_commit(bar_empty + 8 * st);
                     tc_commit(bar_tfull + 8 * (NH * b + hf));           // accumulator part ready
                 }
                 __syncwarp();
             }
-            st += 2;
-            if (st >= kStages) { st -= kStages; fph ^= 1u; }
         }
     } else {
-        // ===== epilogue: set e handles tiles i with (i & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
+        // ===== epilogue: set e drains the items w with (w & 1) == e; warp quarter q owns TMEM lanes 32q.. =====
         const int e = (warp - 2) >> 2, q = warp & 3;
         float sse32 = 0.f, comp = 0.f;
         const int r0 = (npos & 31) ? (npos & 31) : (npos > 0 ? 32 : 0);   // non-negative units in chunk 0
         f32x2 sgn0[16];                                                  // +-1 weights of chunk 0
 #pragma unroll
         for (int t = 0; t < 16; ++t) sgn0[t] = pack2(2 * t < r0 ? 1.f : -1.f, 2 * t + 1 < r0 ? 1.f : -1.f);
-        for (uint32_t i = e; i < nt; i += 2) {
+        float yp = 0.f, yv = 0.f;
+        for (uint32_t w = e, kth = 0; w < nitems; w += 2, ++kth) {
+            const uint32_t i = w / NS, sl = w % NS;
             const long long row = (blockIdx.x + (long long)i * gridDim.x) * kTile + q * 32 + lane;
-            const float yv = row < n ? __ldg(Y + row) : 0.f;
-            float yp = 0.f;
+            if (sl < 2) {                                       // first slice this set takes from the tile
+                yp = 0.f;
+                yv = ((NS == 1 || e == 0) && row < n) ? __ldg(Y + row) : 0.f;
+            }
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) {
-                mbar_wait(bar_tfull + 8 * (NH * e + hf), (unsigned)(i >> 1) & 1u);
+                mbar_wait(bar_tfull + 8 * (NH * e + hf), kth & 1u);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + e * 256 + hf * CP;
                 uint32_t z[2][32];
@@ -239,23 +257,31 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
 #pragma unroll
                 for (int c = 0; c < CP / 32; ++c) {
                     if (c + 1 < CP / 32) tmem_ld32(taddr + (c + 1) * 32, z[(c + 1) & 1]);
-                    const int cb = hf * CP + c * 32;                            // first (permuted) column
+                    const int cb = (int)sl * HS + hf * CP + c * 32;             // first (permuted) column
                     const float* zc = reinterpret_cast<const float*>(z[c & 1]);
+                    // chunk 0 of the permuted order (columns 0..31) holds both signs
+                    const bool mixed = hf == 0 && c == 0 && (NS == 1 || sl == 0);
                     f32x2 sc[4];
+                    if (hf == 0 && c == 0 && mixed) {
 #pragma unroll
-                    for (int t = 0; t < 32; t += 2) {                           // eq. 2 on two pipes
-                        const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
-                        const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
-                        const int a4 = (t >> 1) & 3;
-                        if (hf == 0 && c == 0) {                                // chunk 0: signed sum
+                        for (int t = 0; t < 32; t += 2) {                       // signed sum
+                            const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
+                            const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
+                            const int a4 = (t >> 1) & 3;
                             if (t < 8) sc[a4] = fmul2(pack2(h0, h1), sgn0[t >> 1]);
                             else ffma2(sc[a4], pack2(h0, h1), sgn0[t >> 1]);
-                        } else {
+                        }
+                    } else {
+#pragma unroll
+                        for (int t = 0; t < 32; t += 2) {                       // eq. 2 on two pipes
+                            const float h0 = t < 24 ? fmaxf(zc[t], 0.f) : zc[t] + fabsf(zc[t]);
+                            const float h1 = t < 24 ? fmaxf(zc[t + 1], 0.f) : zc[t + 1] + fabsf(zc[t + 1]);
+                            const int a4 = (t >> 1) & 3;
                             sc[a4] = t < 8 ? pack2(h0, h1) : fadd2(sc[a4], pack2(h0, h1));
                         }
                     }
                     const float csum = hsum2(fadd2(fadd2(sc[0], sc[1]), fadd2(sc[2], sc[3])));
-                    if (hf == 0 && c == 0) yp += csum;                           // signs applied per column
+                    if (mixed) yp += csum;                                       // signs applied per column
                     else yp = fmaf(cb - 32 < npos - r0 ? 1.f : -1.f, csum, yp);  // eq. 3: sign of the chunk
                     if (c + 1 < CP / 32) tmem_ld_wait();
                     if (c + 2 == CP / 32 || CP == 32) {
@@ -265,6 +291,15 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
                         if (lane == 0) mbar_arrive(bar_tempty + 8 * (NH * e + hf));
                     }
                 }
+            }
+            if (sl + 2 < NS) continue;                          // more slices of this tile for this set
+            if constexpr (NS > 1) {
+                // the two sets hold the two halves of the row sum: set 1 hands its half to set 0
+                float* rp = rowpart + (i & 1u) * kTile + q * 32 + lane;
+                if (e == 1) *rp = yp;
+                asm volatile("bar.sync %0, 64;" ::"r"(1 + q) : "memory");
+                if (e == 0) yp += *rp;
+                if (e == 1) continue;
             }
             const float err = row < n ? yp - yv : 0.f;
             const float t = fmaf(err, err, -comp);                             // eq. 4, Kahan-compensated fp32
@@ -323,7 +358,7 @@ template <int H>
 cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const float* W1, const float* W2,
                      double* partials, int grid, double* d_out, cudaStream_t stream) {
     auto kern = k_eval_tf32<H>;
-    const size_t smem = (size_t)H * kIn * 4 + (size_t)kStages * kTileBytes + (size_t)H * 4 +
+    const size_t smem = (size_t)H * kIn * 4 + (size_t)eval_stages(H) * kTileBytes + (size_t)H * 4 + 2 * kTile * 4 + 32 * 4 +
                         8 * (2 * kStages + 16) + 8 * 8 + 4 * H + 32 + 4 + 16;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
@@ -335,7 +370,7 @@ cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const
 }  // namespace
 
 bool eval_tf32_supported(int hidden) {
-    return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256;
+    return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256 || hidden == 512 || hidden == 1024;
 }
 
 cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
@@ -361,6 +396,8 @@ cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const fl
         case 64: err = launch_h<64>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
         case 128: err = launch_h<128>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
         case 256: err = launch_h<256>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
+        case 512: err = launch_h<512>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
+        case 1024: err = launch_h<1024>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
         default: return cudaErrorInvalidValue;
     }
     if (err == cudaSuccess) ++*launches;
