@@ -5,27 +5,29 @@
 // the cluster: CTA c owns S = hidden/C hidden units, i.e. W1[:, cS:(c+1)S] and W2[cS:(c+1)S],
 // whose fp32 master copy stays in shared memory for the whole run.
 //
-// Mapping inside a CTA (8 warps), v2:
-//   * a lane owns FOUR hidden units (u_j = lu + j*LPS, lu = lane % LPS, LPS = S/4).  During the
-//     forward pass it holds their W1 columns (4 x 32 floats) in registers, during the backward
-//     pass the same registers hold the dW1 accumulators: the two live ranges never overlap, so a
-//     128-bit shared-memory load of X feeds 8 FFMA2 (fma.rn.f32x2) instead of v1's 4 -- on
-//     sm_100a an LDS.128 costs 2 cycles of the SM's shared-memory pipe, 8 FFMA2 cost 4 cycles of
-//     the FMA pipes, so the FMA pipe is the binding unit (profiles/r01_ncu_v1.md);
-//   * a warp instruction covers SPW = 32/LPS rows (one per lane sub-group s = lane / LPS).  The
-//     X tile is stored as SPW blocks of BT/SPW rows, block s shifted by 16*s bytes, so the SPW
-//     rows read by one LDS.128 fall into distinct bank groups (no conflict, no swizzle);
-//   * H = ReLU(Z1) of the warp's rows stays in registers between forward and backward.
-// Per tile: forward (eqs. 1-3) -> per-row partial Ypred reduced across the LPS lanes with a
-// transposing shuffle tree -> pushed to every CTA of the cluster with st.async (DSMEM store that
-// completes transaction bytes on the destination's mbarrier: one hop, no flag) -> every CTA sums
-// the C partials in rank order -> dZ2 (eq. 5) -> dW2, dZ1, dW1 (eqs. 6-8) accumulated in
-// registers.  The tile is processed as NSPLIT row groups so that the exchange of one group is in
-// flight while the other group computes.  After the backward pass the SPW sub-groups' partial
-// dW1 are combined with a transposing butterfly (each lane ends with 1/SPW of the sums), added
-// to the warp's shared-memory partial; at the end of the batch the 8 warps' partials are summed
-// in a fixed order (deterministic), eq. 9 is applied to the shared-memory master copy.
-// X tiles arrive by cp.async.bulk (TMA engine) into a 3-stage ring, one tile ahead.
+// Mapping inside a CTA (8 warps):
+//   * a lane owns FOUR hidden units (u_j = lu + j*LPS, lu = lane % LPS, LPS = S/4); a warp
+//     instruction covers SPW = 32/LPS rows (one per lane sub-group s = lane / LPS).  The X tile is
+//     stored as SPW blocks of BT/SPW rows, block s shifted by 16*s bytes, so the SPW rows read by
+//     one LDS.128 fall into distinct bank groups (no conflict, no swizzle);
+//   * forward (eqs. 1-3): the lane's four W1 columns (4 x 32 floats) live in registers for the
+//     forward pass only; one 128-bit shared-memory load of X feeds 8 FFMA2 (fma.rn.f32x2).  The
+//     first row group is processed chunk-major so the register reload of W1 (4 shared-memory
+//     cycles per LDS.128: ~1,000 cycles per CTA) overlaps its FMAs.  H = ReLU(Z1) of the warp's
+//     rows stays in registers between forward and backward;
+//   * per-row partial Ypred: transposing shuffle tree over the LPS lanes, then pushed to every CTA
+//     of the cluster with st.async (DSMEM store that completes transaction bytes on the
+//     destination's mbarrier: one hop, no flag), one fixed peer per lane, straight-line code (the
+//     cluster size is a template parameter).  The tile is processed as NSPLIT row groups so that
+//     the exchange of one group is in flight while the other group computes;
+//   * backward (eqs. 5-8), K-split: every CTA sums the C partials (fixed tree) -> dZ2; the lane of
+//     sub-group s accumulates dW1 only for inputs [IPS*s, IPS*(s+1)) of its four units (32
+//     registers at SPW = 4) but over the rows of ALL sub-groups, whose dZ1 arrives by shuffle: no
+//     reduction across sub-groups.  Per-warp partials go to shared memory; at the end of the batch
+//     the 8 warps' partials are summed by a fixed pairwise tree (deterministic) and eq. 9 is
+//     applied to the shared-memory master copy.
+// X tiles arrive by cp.async.bulk (TMA engine) into a 3-stage ring, one tile ahead; Y one tile
+// ahead into a holder lane's register.  Measured: DESIGN.md 5.1, profiles/r01_ncu_v3.md.
 #include "common.cuh"
 #include "internal.h"
 
