@@ -95,6 +95,18 @@ int mlp_train_ex(const float* X, const float* Y, int64_t n, int batch, float lr,
                  float* W1, float* W2, const int32_t* batch_order, int variant, void* stream);
 
 /*
+ * mlp_train_rows -- mini-batch SGD with SAMPLE-level shuffling (the other reading of "batch order",
+ * DESIGN.md reading 5; the paper is silent on shuffling): in epoch e, batch k is
+ * rows row_order[e*n + k*batch .. e*n + min(n, (k+1)*batch)) of X/Y.
+ *   row_order: DEVICE int32 [epochs*n], each epoch a permutation of 0..n-1 (not validated).
+ * Per epoch the rows are gathered into library-owned scratch (one pass at HBM speed) and the fused
+ * kernel runs the epoch on the gathered copy: two launches per epoch.  Same arithmetic, same
+ * error behaviour and asynchrony as mlp_train; the scratch (n*132 bytes) is freed by mlp_shutdown.
+ */
+int mlp_train_rows(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
+                   float* W1, float* W2, const int32_t* row_order, void* stream);
+
+/*
  * mlp_eval_loss -- eq. 4 over the whole dataset:
  *   L = (1/n) sum_r (ReLU(X_r W1) W2 - Y_r)^2.
  * Synchronises `stream` and returns L; NaN on error (then see mlp_last_error()).

@@ -24,7 +24,7 @@ VARIANT_PRIOR_TILED = 4
 EXPORTS = [
     "mlp_init", "mlp_init_weights", "mlp_train", "mlp_train_ex", "mlp_eval_loss",
     "mlp_eval_loss_async", "mlp_train_host", "mlp_eval_loss_host", "mlp_set_cluster",
-    "mlp_get_cluster", "mlp_get_train_stats", "mlp_launch_count", "mlp_last_error",
+    "mlp_train_rows", "mlp_get_cluster", "mlp_get_train_stats", "mlp_launch_count", "mlp_last_error",
     "mlp_version", "mlp_shutdown",
 ]
 
@@ -53,6 +53,7 @@ def lib():
     L.mlp_train.argtypes = [vp, vp, i64, i32, f32, i32, vp, vp, vp]; L.mlp_train.restype = i32
     L.mlp_train_ex.argtypes = [vp, vp, i64, i32, f32, i32, vp, vp, vp, i32, vp]
     L.mlp_train_ex.restype = i32
+    L.mlp_train_rows.argtypes = [vp, vp, i64, i32, f32, i32, vp, vp, vp, vp]; L.mlp_train_rows.restype = i32
     L.mlp_eval_loss.argtypes = [vp, vp, i64, vp, vp, vp]; L.mlp_eval_loss.restype = f64
     L.mlp_eval_loss_async.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp]
     L.mlp_eval_loss_async.restype = i32
@@ -112,6 +113,13 @@ def mlp_train_ex(X, Y, n, batch, lr, epochs, W1, W2, batch_order=None, variant=V
     _check(lib().mlp_train_ex(_dptr(X, "float32", "X"), _dptr(Y, "float32", "Y"), int(n), int(batch),
                               float(lr), int(epochs), _dptr(W1, "float32", "W1"),
                               _dptr(W2, "float32", "W2"), op, int(variant), _stream(stream)))
+
+
+def mlp_train_rows(X, Y, n, batch, lr, epochs, W1, W2, row_order, stream=None) -> None:
+    _check(lib().mlp_train_rows(_dptr(X, "float32", "X"), _dptr(Y, "float32", "Y"), int(n), int(batch),
+                                float(lr), int(epochs), _dptr(W1, "float32", "W1"),
+                                _dptr(W2, "float32", "W2"), _dptr(row_order, "int32", "row_order"),
+                                _stream(stream)))
 
 
 def mlp_eval_loss(X, Y, n, W1, W2, stream=None) -> float:

@@ -27,6 +27,7 @@ struct State {
     unsigned long long* stats = nullptr;
     UnfusedScratch unf = {};          int unf_batch = 0, unf_hidden = 0;
     float *priorXT = nullptr, *priorHT = nullptr;   // transposes of the paper's tiled strategy
+    float *shufX = nullptr, *shufY = nullptr; size_t shufX_cap = 0, shufY_cap = 0;   // mlp_train_rows
     float *hX = nullptr, *hY = nullptr, *hW1 = nullptr, *hW2 = nullptr; int32_t* hOrder = nullptr;
     size_t hX_cap = 0, hY_cap = 0, hW_cap = 0, hOrder_cap = 0;
     cudaStream_t host_stream = nullptr;
@@ -271,6 +272,24 @@ int mlp_eval_loss_async(const float* X, const float* Y, int64_t n, const float* 
     return eval_impl(X, Y, n, W1, W2, d_out, variant, (cudaStream_t)stream);
 }
 
+int mlp_train_rows(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
+                   float* W1, float* W2, const int32_t* row_order, void* stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!row_order) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
+    int rc = check_train_args(X, Y, n, batch, lr, epochs, W1, W2, MLP_VARIANT_FUSED);
+    if (rc) return rc;
+    if (n > 0x7fffffffLL / 8) return fail(MLP_ERR_BAD_ARG, "n too large for int32 row indices");
+    if ((rc = grow(&g.shufX, &g.shufX_cap, (size_t)n * kIn))) return rc;
+    if ((rc = grow(&g.shufY, &g.shufY_cap, (size_t)n))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int e = 0; e < epochs; ++e) {
+        cudaError_t err = launch_gather_rows(X, Y, row_order + (int64_t)e * n, g.shufX, g.shufY, n, st, &g.launches);
+        if (err != cudaSuccess) return cuda_fail(err, "launch_gather_rows");
+        if ((rc = train_impl(g.shufX, g.shufY, n, batch, lr, 1, W1, W2, nullptr, MLP_VARIANT_FUSED, st))) return rc;
+    }
+    return MLP_OK;
+}
+
 int mlp_train_host(const float* X_host, const float* Y_host, int64_t n, int batch, float lr,
                    int epochs, float* W1_host, float* W2_host, const int32_t* order_host,
                    int variant) {
@@ -355,7 +374,7 @@ const char* mlp_version(void) { return "libmlp_b200 0.1 (sm_100a)"; }
 void mlp_shutdown(void) {
     std::lock_guard<std::mutex> lk(g_mu);
     void* ptrs[] = {g.eval_partials, g.eval_out, g.stats, g.unf.Z1, g.unf.Hact, g.unf.dZ1,
-                    g.unf.Ypred, g.unf.dZ2, g.unf.dW1, g.unf.dW2, g.priorXT, g.priorHT, g.hX, g.hY, g.hW1, g.hOrder};
+                    g.unf.Ypred, g.unf.dZ2, g.unf.dW1, g.unf.dW2, g.priorXT, g.priorHT, g.shufX, g.shufY, g.hX, g.hY, g.hW1, g.hOrder};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (g.host_stream) cudaStreamDestroy(g.host_stream);
     const bool init = g.init; const uint64_t seed = g.seed;

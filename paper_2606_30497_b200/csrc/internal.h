@@ -33,6 +33,8 @@ cudaError_t launch_train_prior(bool tiled, const float* X, const float* Y, int64
                                int epochs, float* W1, float* W2, const int32_t* order_host, int hidden,
                                const UnfusedScratch& s, float* XT, float* HT, cudaStream_t stream,
                                int64_t* launches);
+cudaError_t launch_gather_rows(const float* X, const float* Y, const int32_t* perm, float* Xp, float* Yp,
+                               int64_t n, cudaStream_t stream, int64_t* launches);
 cudaError_t launch_init_weights(uint64_t seed, int hidden, float* W1, float* W2,
                                 cudaStream_t stream, int64_t* launches);
 

@@ -92,7 +92,29 @@ __global__ void k_init_weights(unsigned long long seed, int H, float* __restrict
     if (e < n1) W1[e] = w; else W2[e - n1] = w;
 }
 
+// sample-level shuffling: Xp[r] = X[perm[r]], Yp[r] = Y[perm[r]]; one
+// float4 per thread, eight threads per 128-byte row
+__global__ void k_gather_rows(const float* __restrict__ X, const float* __restrict__ Y,
+                              const int* __restrict__ perm, float* __restrict__ Xp,
+                              float* __restrict__ Yp, long long n) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long r = e >> 3;
+    if (r >= n) return;
+    const int c = (int)(e & 7);
+    const long long src = perm[r];
+    reinterpret_cast<float4*>(Xp)[e] = __ldg(reinterpret_cast<const float4*>(X) + src * 8 + c);
+    if (c == 0) Yp[r] = __ldg(Y + src);
+}
+
 }  // namespace
+
+cudaError_t launch_gather_rows(const float* X, const float* Y, const int32_t* perm, float* Xp, float* Yp,
+                               int64_t n, cudaStream_t stream, int64_t* launches) {
+    const long long total = (long long)n * 8;
+    k_gather_rows<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(X, Y, perm, Xp, Yp, n);
+    ++*launches;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_init_weights(uint64_t seed, int hidden, float* W1, float* W2,
                                 cudaStream_t stream, int64_t* launches) {

@@ -102,6 +102,13 @@ def make_order(n: int, batch: int, epochs: int, shuffle: bool, seed: int = 3):
     return np.stack([rp.permutation(nb) for _ in range(epochs)]).astype(np.int32)
 
 
+def make_row_order(n: int, epochs: int, seed: int = 3):
+    """Sample-level shuffling: one permutation of the n rows per epoch, int32
+    [epochs x n], drawn from numpy default_rng(seed)."""
+    rp = np.random.default_rng(seed)
+    return np.stack([rp.permutation(n) for _ in range(epochs)]).astype(np.int32)
+
+
 def numpy_init_weights(hidden: int, seed: int = 2):
     """U(+-1/sqrt(fan_in)) from numpy's generator -- used ONLY by pin P14 (SURVEY.md
     8(c)); the library's own init is the counter-based generator of include/mlp.h."""

@@ -113,6 +113,23 @@ def test_paper_strategies_match_oracle(variant, hidden, batch, n):
     assert nerr(g1, o1) <= 1e-5 and nerr(g2, o2) <= 1e-5, (variant, nerr(g1, o1), nerr(g2, o2))
 
 
+# Sample-level shuffling: the oracle sees the physically permuted epoch.
+@pytest.mark.parametrize("hidden,batch,n,epochs", [(256, 256, 4096, 2), (64, 100, 1001, 3), (256, 300, 70001, 1)])
+def test_train_rows_sample_level_shuffle(hidden, batch, n, epochs):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(2, 32, hidden)
+    rows = datagen.make_row_order(n, epochs)
+    o1, o2 = W1, W2
+    for e in range(epochs):
+        o1, o2 = O.train(np.ascontiguousarray(X[rows[e]]), np.ascontiguousarray(Y[rows[e]]), o1, o2, batch, LR, 1)
+    B.mlp_init(2, 32, hidden, 1)
+    dX, dY, d1, d2 = dev(X), dev(Y), dev(W1), dev(W2)
+    B.mlp_train_rows(dX, dY, n, batch, LR, epochs, d1, d2, dev(rows.reshape(-1)))
+    torch.cuda.synchronize()
+    assert nerr(d1.cpu().numpy(), o1) <= 1e-5 and nerr(d2.cpu().numpy(), o2) <= 1e-5
+    assert torch.equal(dX, dev(X)) and torch.equal(dY, dev(Y))            # inputs untouched
+
+
 # ------------------------------------------------------------------ config 2 (shuffled batch order)
 def test_config2_epoch_and_final_loss():
     c = datagen.CONFIGS["config2"]
