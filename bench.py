@@ -323,6 +323,29 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     unfused_us = a.elapsed_time(b) * 1e3 / datagen.num_batches(cfg.n, cfg.batch)
 
+    # ---- tensor-core training variant (TF32 forward; separately reported, own tolerance) ----
+    tc = None
+    try:
+        tst = []
+        for _ in range(3):
+            t1, t2 = W1i.clone(), W2i.clone()
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            B.mlp_train_ex(dX, dY, cfg.n, cfg.batch, cfg.lr, cfg.epochs, t1, t2, dO, B.VARIANT_TF32)
+            b.record()
+            torch.cuda.synchronize()
+            tst.append(a.elapsed_time(b))
+        B.mlp_eval_loss_async(dX, dY, cfg.n, t1, t2, dloss, B.VARIANT_FUSED)
+        torch.cuda.synchronize()
+        ltc = float(dloss.item())
+        tc = {"us_per_sgd_step": min(tst) * 1e3 / sgd_steps, "samples_per_s": samples_per_step / (min(tst) * 1e-3),
+              "final_loss": ltc, "final_loss_rel_diff_vs_fp32_path": abs(ltc - final_loss) / final_loss,
+              "max_rel_weight_diff_vs_fp32_path": float(((t1 - d1).abs().max() / d1.abs().max()).item()),
+              "stated_tolerance": "weights 5e-5 after 1 step, 2e-3 after 1 epoch, loss 1 % (vs the oracle)"}
+    except B.MlpError:
+        pass
+
     # ---- concurrent replicas: R independent models of the same job on R streams,
     #      each a cluster of `cluster` SMs; aggregate samples/s over all models ----
     conc = {}
@@ -392,7 +415,7 @@ def run_ours(args, rank, world, local_rank):
         "us_per_sgd_step": us_per_sgd, "final_loss": final_loss,
         "roofline": roof, "train_by_cluster": by_cluster, "eval_4M_rows": best, "e2e": e2e, "e2e_bitwise_equal_to_device_path": e2e_matches,
         "gpu_launches": int(launches), "unfused_baseline_us_per_sgd_step": unfused_us,
-        "concurrent_replicas": conc, "paper_shapes": paper_shapes, "cpu_baseline": cpu, "clocks": sampler.summary(),
+        "train_tf32_variant": tc, "concurrent_replicas": conc, "paper_shapes": paper_shapes, "cpu_baseline": cpu, "clocks": sampler.summary(),
         "context": "paper (Tesla T4, optimised kernels): 1,482 us/step, 172.7 k samples/s (PAPER.md:330, derived)",
     }
     print(json.dumps(line))

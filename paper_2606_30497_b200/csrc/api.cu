@@ -114,7 +114,7 @@ int check_train_args(const float* X, const float* Y, int64_t n, int batch, float
     if (batch < 1) return fail(MLP_ERR_BAD_ARG, "batch must be >= 1 (got %d)", batch);
     if (epochs < 0) return fail(MLP_ERR_BAD_ARG, "epochs must be >= 0 (got %d)", epochs);
     if (!std::isfinite(lr)) return fail(MLP_ERR_BAD_ARG, "lr must be finite");
-    if (variant != MLP_VARIANT_FUSED && variant != MLP_VARIANT_UNFUSED &&
+    if (variant != MLP_VARIANT_FUSED && variant != MLP_VARIANT_UNFUSED && variant != MLP_VARIANT_TF32 &&
         variant != MLP_VARIANT_PRIOR_NAIVE && variant != MLP_VARIANT_PRIOR_TILED)
         return fail(MLP_ERR_UNSUPPORTED, "training variant %d is not supported", variant);
     if (((uintptr_t)X & 15) || ((uintptr_t)W1 & 15))
@@ -144,6 +144,13 @@ int train_impl(const float* X, const float* Y, int64_t n, int batch, float lr, i
         cudaError_t e = launch_train_fused(X, Y, n, batch, lr, epochs, W1, W2, order, g.hidden, C,
                                            g.stats, stream, &g.launches);
         if (e != cudaSuccess) return cuda_fail(e, "launch_train_fused");
+        return MLP_OK;
+    }
+    if (variant == MLP_VARIANT_TF32) {
+        if (!train_tf32_supported(g.hidden))
+            return fail(MLP_ERR_UNSUPPORTED, "TF32 training variant needs hidden 256 (got %d)", g.hidden);
+        cudaError_t e = launch_train_tf32(X, Y, n, batch, lr, epochs, W1, W2, order, g.hidden, stream, &g.launches);
+        if (e != cudaSuccess) return cuda_fail(e, "launch_train_tf32");
         return MLP_OK;
     }
     // unfused baseline: the host loop needs the batch order on the host

@@ -369,6 +369,18 @@ cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const
 
 }  // namespace
 
+bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows) {
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)kIn, (cuuint64_t)n};
+    const cuuint64_t strides[1] = {(cuuint64_t)kIn * 4};
+    const cuuint32_t box[2] = {(cuuint32_t)kIn, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return enc(static_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(X),
+               dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 bool eval_tf32_supported(int hidden) {
     return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256 || hidden == 512 || hidden == 1024;
 }
@@ -377,19 +389,10 @@ cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const fl
                              int hidden, double* partials, int grid, double* d_out, cudaStream_t stream,
                              int64_t* launches) {
     if (n > 0x7fffffffLL - kTile) return cudaErrorInvalidValue;      // TMA coordinates are int32
-    EncodeTiledFn enc = encode_tiled();
-    if (!enc) return cudaErrorNotSupported;
     // X as a 2-D tensor [n rows][32 floats]; box = one 128-row tile; 128-byte swizzle = the layout
     // tcgen05.mma reads a K-major operand in (a row is exactly one 128-byte swizzle span).
     CUtensorMap tmap;
-    const cuuint64_t dims[2] = {(cuuint64_t)kIn, (cuuint64_t)n};
-    const cuuint64_t strides[1] = {(cuuint64_t)kIn * 4};
-    const cuuint32_t box[2] = {(cuuint32_t)kIn, (cuuint32_t)kTile};
-    const cuuint32_t estr[2] = {1, 1};
-    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(X), dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return cudaErrorInvalidValue;
+    if (!make_x_tensormap(&tmap, X, n, kTile)) return cudaErrorNotSupported;
     cudaError_t err;
     switch (hidden) {
         case 32: err = launch_h<32>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;

@@ -44,6 +44,17 @@ cudaError_t launch_eval_fp32(const float* X, const float* Y, int64_t n, const fl
                              const float* W2, int hidden, double* partials, int grid,
                              double* d_out, cudaStream_t stream, int64_t* launches);
 
+// X viewed as a 2-D tensor [n][32] fp32 with 128-byte swizzle, box = box_rows rows (<= 256); *out_map is a
+// CUtensorMap (128 bytes, 64-byte aligned).  False if the driver entry point is unavailable.
+bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows);
+
+// train_tf32.cu -- fused cluster training kernel with eq. 1 on the tensor cores (row a-T, separately
+// reported; hidden 256 on a cluster of 8 only)
+bool train_tf32_supported(int hidden);
+cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
+                              float* W1, float* W2, const int32_t* order, int hidden,
+                              cudaStream_t stream, int64_t* launches);
+
 // eval_tf32.cu -- tcgen05 TF32 first layer (row a-T, separately reported)
 bool eval_tf32_supported(int hidden);
 cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const float* W1,

@@ -130,6 +130,37 @@ def test_train_rows_sample_level_shuffle(hidden, batch, n, epochs):
     assert torch.equal(dX, dev(X)) and torch.equal(dY, dev(Y))            # inputs untouched
 
 
+# Tensor-core training variant (TF32 forward): separately reported, stated
+# tolerance 5e-5 after one step, 2e-3 after one epoch, loss within 1 %.
+def test_train_tf32_variant_one_step_and_epoch(cfg1):
+    X, Y, W1, W2 = cfg1
+    g1, g2 = gpu_train(X[:256], Y[:256], W1, W2, 256, LR, 1, variant=B.VARIANT_TF32)
+    o1, o2 = O.train(X[:256], Y[:256], W1, W2, 256, LR, 1)
+    assert nerr(g1, o1) <= 5e-5 and nerr(g2, o2) <= 5e-5, (nerr(g1, o1), nerr(g2, o2))
+    c = datagen.CONFIGS["config2"]
+    X, Y = datagen.make_dataset(c.n, c.sigma)
+    order = datagen.make_order(c.n, c.batch, c.epochs, True)
+    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1], variant=B.VARIANT_TF32)
+    o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1])
+    assert nerr(g1, o1) <= 2e-3 and nerr(g2, o2) <= 2e-3, (nerr(g1, o1), nerr(g2, o2))
+    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order, variant=B.VARIANT_TF32)
+    o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order)
+    lg, lo = gpu_eval(X, Y, g1, g2), O.eval_loss(X, Y, o1, o2)
+    assert abs(lg - lo) <= 1e-2 * lo, (lg, lo)
+
+
+@pytest.mark.parametrize("batch,n", [(32, 2048), (1024, 8192), (100, 1001), (300, 1000), (5000, 3000), (1, 7)])
+def test_train_tf32_variant_batches_and_ragged(batch, n):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(2, 32, 256)
+    order = datagen.make_order(n, batch, 2, True)
+    o1, o2 = O.train(X, Y, W1, W2, batch, LR, 2, order=order)
+    g1, g2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=B.VARIANT_TF32)
+    assert nerr(g1, o1) <= 2e-3 and nerr(g2, o2) <= 2e-3, (batch, n, nerr(g1, o1), nerr(g2, o2))
+    h1, h2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=B.VARIANT_TF32)
+    assert np.array_equal(g1, h1) and np.array_equal(g2, h2)              # deterministic
+
+
 # ------------------------------------------------------------------ config 2 (shuffled batch order)
 def test_config2_epoch_and_final_loss():
     c = datagen.CONFIGS["config2"]
