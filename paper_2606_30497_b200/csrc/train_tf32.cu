@@ -103,7 +103,8 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     unsigned char* Xs = smem;                                             // [kRing][32 KB] swizzled rows
     unsigned char* Wop = Xs + kRing * kXBytes;                            // [S][128 B] B operand (K-major, swizzled)
     unsigned char* Hs = Wop + S * 128;                                    // [BT][128 B] H = ReLU(Z1), swizzled rows
-    float* part = reinterpret_cast<float*>(Hs + BT * 128);                // [kWarps][S*32]  layout [q][slot][4]
+    unsigned char* Ms = Hs + BT * 128;                                    // [BT][128 B] ReLU'(Z1) * W2 (eq. 7 factor), swizzled
+    float* part = reinterpret_cast<float*>(Ms + BT * 128);                // [kWarps][S*32]  layout [q][slot][4]
     float* W1m = part + kWarps * S * kIn;                                 // [S*32] fp32 master, layout [q][slot][4]
     float* ypp = W1m + S * kIn;                                           // [2][C][BT]
     float* part2 = ypp + 2 * C * BT;                                      // [kWarps][S]
@@ -169,7 +170,6 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     const uint32_t ypp_a = smem_u32(ypp), yp_a = bar_yp;
     const int rowl = warp * ITER;
     float* mypart = part + warp * (S * kIn);
-    float w2r[4];                                              // backward: lane owns units 4*lu .. 4*lu+3
 
     constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(S >> 3) << 17) |
                                ((uint32_t)(128 >> 4) << 24);
@@ -182,8 +182,6 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
         const int ntiles = (m + BT - 1) / BT;
         const float scale = t_cur == p.nbi - 1 ? p.scale_last : p.scale_full;   // eq. 5: 2 / m
         float g2[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-        for (int u = 0; u < 4; ++u) w2r[u] = W2s[4 * lu + u];
 
         for (int j = 0; j < ntiles; ++j, ++gt) {
             const unsigned buf = gt & 1u, ph = (gt >> 1) & 1u;
@@ -237,6 +235,8 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                     h.x = fmaxf(__uint_as_float(z[4 * c]), 0.f);      h.y = fmaxf(__uint_as_float(z[4 * c + 1]), 0.f);   // eq. 2
                     h.z = fmaxf(__uint_as_float(z[4 * c + 2]), 0.f);  h.w = fmaxf(__uint_as_float(z[4 * c + 3]), 0.f);
                     *reinterpret_cast<float4*>(Hs + swz(frow, c)) = h;
+                    *reinterpret_cast<float4*>(Ms + swz(frow, c)) =                       // eq. 7: ReLU'(z) w2 (old W2)
+                        make_float4(h.x > 0.f ? w.x : 0.f, h.y > 0.f ? w.y : 0.f, h.z > 0.f ? w.z : 0.f, h.w > 0.f ? w.w : 0.f);
                     pr[c & 3] = fmaf(h.x, w.x, fmaf(h.y, w.y, fmaf(h.z, w.z, fmaf(h.w, w.w, pr[c & 3]))));   // eq. 3
                 }
                 const float pv = (pr[0] + pr[1]) + (pr[2] + pr[3]);
@@ -271,13 +271,17 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 for (int t = 0; t < SPW; ++t) {
                     const int r = (s ^ t) * RB + rowl + it;                    // tile row
                     const float d = Ds[r];
-                    const float4 h = *reinterpret_cast<const float4*>(Hs + swz(r, lu));
-                    const float hh[4] = {h.x, h.y, h.z, h.w};
+                    const float4 mk = *reinterpret_cast<const float4*>(Ms + swz(r, lu));
+                    const float mm[4] = {mk.x, mk.y, mk.z, mk.w};
+                    if (t == 0) {                                              // eq. 6 (each row once per CTA)
+                        const float4 h = *reinterpret_cast<const float4*>(Hs + swz(r, lu));
+                        g2[0] = fmaf(h.x, d, g2[0]); g2[1] = fmaf(h.y, d, g2[1]);
+                        g2[2] = fmaf(h.z, d, g2[2]); g2[3] = fmaf(h.w, d, g2[3]);
+                    }
                     f32x2 dd[4];
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
-                        if (t == 0) g2[u] = fmaf(hh[u], d, g2[u]);             // eq. 6 (each row once per CTA)
-                        const float e = hh[u] > 0.f ? d * w2r[u] : 0.f;        // eq. 7 (old W2)
+                        const float e = d * mm[u];                             // eq. 7
                         dd[u] = pack2(e, e);
                     }
 #pragma unroll
@@ -392,7 +396,7 @@ cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int bat
     if (p.total_steps == 0) return cudaSuccess;
     alignas(64) CUtensorMap tmap;
     if (!make_x_tensormap(&tmap, X, n, kBT)) return cudaErrorNotSupported;
-    const size_t smem = (size_t)kRing * kXBytes + kS * 128 + kBT * 128 +
+    const size_t smem = (size_t)kRing * kXBytes + kS * 128 + 2 * kBT * 128 +
                         sizeof(float) * (kWarps * kS * kIn + kS * kIn + 2 * kC * kBT + kWarps * kS + kS + kBT) +
                         8 * (2 * kRing + 3) + 16;
     cudaError_t err = cudaFuncSetAttribute(k_train_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
