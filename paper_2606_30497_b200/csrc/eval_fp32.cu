@@ -70,6 +70,8 @@ k_eval_fp32(const float* __restrict__ X, const float* __restrict__ Y, long long 
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kStages);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    __shared__ int last_flag_s;
+    int* last_flag = &last_flag_s;
     const int g = tid / LPS;                 // row group of this thread
     const int gl = tid % LPS;                // lane index inside the group -> hidden units
     const int lu = lane % LW;                // lane index inside the warp's part of the group
@@ -175,11 +177,18 @@ k_eval_fp32(const float* __restrict__ X, const float* __restrict__ Y, long long 
         partials[blockIdx.x] = tot;
         __threadfence();
         const unsigned prev = atomicAdd(ticket, 1u);
-        if (prev == gridDim.x - 1) {
-            __threadfence();
-            double all = 0.0;
-            for (unsigned b = 0; b < gridDim.x; ++b) all += ((volatile double*)partials)[b];
-            *out = all / (double)n;
+        *last_flag = prev == gridDim.x - 1 ? 1 : 0;
+    }
+    __syncthreads();
+    // last block: fixed-order sum of the per-block partials; the loads of one warp are in flight together
+    // (a one-thread loop would pay one L2 round trip per block)
+    if (*last_flag && warp == 0) {
+        __threadfence();
+        double acc = 0.0;
+        for (unsigned b = lane; b < gridDim.x; b += 32) acc += ((volatile double*)partials)[b];
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+        if (lane == 0) {
+            *out = acc / (double)n;
             *ticket = 0u;
         }
     }

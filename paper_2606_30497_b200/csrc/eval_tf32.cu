@@ -122,6 +122,8 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NW = kEvalThreads / 32;
+    __shared__ int last_flag_s;
+    int* last_flag = &last_flag_s;
 
     // ---- setup -------------------------------------------------------------------------------------
     // W2 is folded into the B operand: column j of Z' = X (W1 diag|W2|) is |w2_j| z_j, and
@@ -131,6 +133,24 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     // 32-column chunk has one sign, except chunk 0, which collects the remainder of both signs and
     // is summed with +-1 weights kept in registers.  Columns 24..31 of every chunk take ReLU as
     // (z + |z|) on the FMA pipe and carry a factor 1/2.
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NS > 1 ? 2 : 1); }
+        for (int b = 0; b < 8; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    const long long ntiles = (n + kTile - 1) / kTile;
+    const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const uint32_t nt = (uint32_t)my_tiles;
+    // the first ring fill does not depend on the weights: start it before the operand set-up below
+    if (warp == 0 && elect_one()) {
+        for (uint32_t i = 0; i < nt && i < (uint32_t)NST; ++i) {
+            const long long row0 = (blockIdx.x + (long long)i * gridDim.x) * kTile;
+            mbar_arrive_expect_tx(bar_full + 8 * i, kTileBytes);        // OOB rows are zero-filled, still counted
+            tma_load_2d(smem_u32(Xring) + i * kTileBytes, &tmapX, 0, (int)row0, bar_full + 8 * i);
+        }
+    }
+    __syncwarp();
     for (int g = warp; g < NG; g += NW) {                      // a warp per group of 32 hidden units
         const unsigned bal = __ballot_sync(0xffffffffu, __ldg(W2 + g * 32 + lane) >= 0.f);
         if (lane == 0) wcnt[g] = __popc(bal);
@@ -160,11 +180,6 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
             *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
                 make_float4(wcol[4 * c] * sc, wcol[4 * c + 1] * sc, wcol[4 * c + 2] * sc, wcol[4 * c + 3] * sc);
     }
-    if (tid == 0) {
-        for (int s = 0; s < NST; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NS > 1 ? 2 : 1); }
-        for (int b = 0; b < 8; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
-        fence_mbar_init();
-    }
     if (warp == 1) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot))
                      : "memory");
@@ -178,19 +193,16 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     const int npos = *npos_s;
     if (smem_u32(smem) & 1023u) __trap();
 
-    const long long ntiles = (n + kTile - 1) / kTile;
-    const long long my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     double sse = 0.0;
-    const uint32_t nt = (uint32_t)my_tiles;
     // Work items: item w = i * NS + sl is slice sl of this CTA's i-th tile; it uses accumulator
     // (w & 1), MMA issuer (w & 1) and epilogue set (w & 1).  nt * NS < 2^31 by the host check.
     const uint32_t nitems = nt * NS;
 
     if (warp == 0) {
         // ===== TMA producer (whole warp runs the loop, one elected lane issues) =====
-        uint32_t st = 0, eph = 1;                       // ring stage, parity of the "empty" phase to wait for
-        for (uint32_t i = 0; i < nt; ++i) {
-            if (i >= NST) mbar_wait(bar_empty + 8 * st, eph);
+        uint32_t st = 0, eph = 0;                       // ring stage, parity of the "empty" phase to wait for
+        for (uint32_t i = NST; i < nt; ++i) {           // tiles 0..NST-1 were issued before the set-up
+            mbar_wait(bar_empty + 8 * st, eph);
             if (elect_one()) {
                 const long long row0 = (blockIdx.x + (long long)i * gridDim.x) * kTile;
                 mbar_arrive_expect_tx(bar_full + 8 * st, kTileBytes);   // OOB rows are zero-filled, still counted
@@ -326,11 +338,18 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
         partials[blockIdx.x] = tot;
         __threadfence();
         const unsigned prev = atomicAdd(ticket, 1u);
-        if (prev == gridDim.x - 1) {
-            __threadfence();
-            double all = 0.0;
-            for (unsigned b = 0; b < gridDim.x; ++b) all += ((volatile double*)partials)[b];
-            *out = all / (double)n;
+        *last_flag = prev == gridDim.x - 1 ? 1 : 0;
+    }
+    __syncthreads();
+    // last block: fixed-order sum of the per-block partials; the loads of one warp are in flight together
+    // (a one-thread loop would pay one L2 round trip per block)
+    if (*last_flag && warp == 0) {
+        __threadfence();
+        double acc = 0.0;
+        for (unsigned b = lane; b < gridDim.x; b += 32) acc += ((volatile double*)partials)[b];
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+        if (lane == 0) {
+            *out = acc / (double)n;
             *ticket = 0u;
         }
     }
