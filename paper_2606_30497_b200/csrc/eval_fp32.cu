@@ -3,7 +3,7 @@
 // L = (1/n) sum_r (ReLU(X_r W1) W2 - Y_r)^2     (eqs. 1-4)
 //
 // Persistent grid (a multiple of the SM count).  Each CTA keeps ALL of W1/W2 in registers
-// (a lane owns two hidden units: 2 x 32 weights as packed fp32x2 pairs, as in train_fused.cu)
+// (a lane owns four hidden units: 4 x 32 weights as packed fp32x2 pairs, as in train_fused.cu)
 // and streams 128-row tiles of X (16 KB, one cp.async.bulk each) through a 4-stage
 // shared-memory ring.  LPS = hidden/2 lanes cooperate on one row; the X row is read with
 // broadcast 128-bit loads and eq. 1 runs on FFMA2.  Per-row partial Ypred values are reduced
@@ -41,7 +41,7 @@ struct LaneReduce {
 
 template <int H>
 struct EvalCfg {
-    static constexpr int LPS = H / 2;                               // lanes per row
+    static constexpr int LPS = H / 4;                               // lanes per row (four hidden units per lane)
     static constexpr int NT = LPS > 256 ? LPS : 256;                // threads per CTA
     static constexpr int G = NT / LPS;                              // row groups per CTA
     static constexpr int WPG = LPS >= 32 ? LPS / 32 : 1;            // warps per row group
@@ -99,14 +99,17 @@ k_eval_fp32(const float* __restrict__ X, const float* __restrict__ Y, long long 
     if (tid == 0)
         for (long long i = 0; i < kStages && i < my_tiles; ++i) issue(i);
 
-    // weights: units u0 = gl, u1 = gl + LPS
-    f32x2 w0[16], w1[16];
+    // weights: units gl + j*LPS, j < 4: one 128-bit load of X then feeds 8 FFMA2 (4 with two units per
+    // lane, where the shared-memory pipe and the FMA pipe saturated together)
+    f32x2 w[4][16];
+    float w2r[4];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        w0[k] = pack2(W1[(size_t)(2 * k) * H + gl], W1[(size_t)(2 * k + 1) * H + gl]);
-        w1[k] = pack2(W1[(size_t)(2 * k) * H + gl + LPS], W1[(size_t)(2 * k + 1) * H + gl + LPS]);
+    for (int j = 0; j < 4; ++j) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+            w[j][k] = pack2(W1[(size_t)(2 * k) * H + gl + j * LPS], W1[(size_t)(2 * k + 1) * H + gl + j * LPS]);
+        w2r[j] = W2[gl + j * LPS];
     }
-    const float w2r0 = W2[gl], w2r1 = W2[gl + LPS];
 
     double sse = 0.0;
     unsigned chunk_par = 0;
@@ -135,15 +138,21 @@ k_eval_fp32(const float* __restrict__ X, const float* __restrict__ Y, long long 
 #pragma unroll
             for (int k = 0; k < CH; ++k) {
                 const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xt + (rbase + k) * kIn);
-                f32x2 a0 = 0ull, a1 = 0ull;
+                f32x2 a[4];
 #pragma unroll
                 for (int x = 0; x < 8; ++x) {
                     const ulonglong2 xv = xrow[x];
-                    ffma2(a0, xv.x, w0[2 * x]); ffma2(a1, xv.x, w1[2 * x]);         // eq. 1
-                    ffma2(a0, xv.y, w0[2 * x + 1]); ffma2(a1, xv.y, w1[2 * x + 1]);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        if (x == 0) a[j] = fmul2(xv.x, w[j][0]);                        // eq. 1
+                        else ffma2(a[j], xv.x, w[j][2 * x]);
+                        ffma2(a[j], xv.y, w[j][2 * x + 1]);
+                    }
                 }
-                const float h0 = fmaxf(hsum2(a0), 0.f), h1 = fmaxf(hsum2(a1), 0.f);   // eq. 2
-                pv[k] = fmaf(h1, w2r1, h0 * w2r0);                                     // eq. 3
+                float h[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) h[j] = fmaxf(hsum2(a[j]), 0.f);             // eq. 2
+                pv[k] = fmaf(h[1], w2r[1], h[0] * w2r[0]) + fmaf(h[3], w2r[3], h[2] * w2r[2]);   // eq. 3
             }
             LaneReduce<CH, LW>::run(pv, lu);
             float yp = pv[0];
