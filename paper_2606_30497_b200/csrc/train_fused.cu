@@ -373,19 +373,24 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             ycur = ynext;
 
             // lane (s, lu) owns the 4-input chunks q = (IPS/4)*s + x of its four units
+            if (j == 0) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+                for (int u = 0; u < 4; ++u)
 #pragma unroll
-                for (int x = 0; x < IPS / 4; ++x) {
-                    const int q = (IPS / 4) * s + x;
-                    ulonglong2* dst = reinterpret_cast<ulonglong2*>(mypart + (q * S + lu + u * LPS) * 4);
-                    f32x2 lo = acc[u][2 * x], hi = acc[u][2 * x + 1];
-                    if (j > 0) {                               // later tiles of a large batch
+                    for (int x = 0; x < IPS / 4; ++x)
+                        *reinterpret_cast<ulonglong2*>(mypart + (((IPS / 4) * s + x) * S + lu + u * LPS) * 4) =
+                            make_ulonglong2(acc[u][2 * x], acc[u][2 * x + 1]);
+            } else {                                           // later tiles of a large batch: accumulate
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int x = 0; x < IPS / 4; ++x) {
+                        ulonglong2* dst =
+                            reinterpret_cast<ulonglong2*>(mypart + (((IPS / 4) * s + x) * S + lu + u * LPS) * 4);
                         const ulonglong2 old = *dst;
-                        lo = fadd2(lo, old.x); hi = fadd2(hi, old.y);
+                        *dst = make_ulonglong2(fadd2(acc[u][2 * x], old.x), fadd2(acc[u][2 * x + 1], old.y));
                     }
-                    *dst = make_ulonglong2(lo, hi);
-                }
+            }
         }
 
         // ---------------- end of batch: reduce partial gradients, eq. 9 ----------------
