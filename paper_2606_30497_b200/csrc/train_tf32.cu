@@ -1,21 +1,25 @@
 // train_tf32.cu -- tensor-core variant of the fused training kernel (SURVEY.md 8(a) row a-T,
 // 8(f) NEXT-2; BASELINE.json: "allowed only as a separately reported variant with its own stated
-// tolerance").  Same method, same loop, same cluster layout as train_fused.cu (eqs. 1-9,
-// PAPER.md:44-71; one launch for every batch of every epoch), but eq. 1 (Z1 = X W1) runs on the
-// tensor cores: per 256-row tile two tcgen05.mma chains (M=128, N=32 hidden units of this CTA,
-// K=32 in four K=8 steps, kind::tf32: fp32 operands truncated to TF32, fp32 accumulate in TMEM).
+// tolerance").  Same method, same loop, same cluster layout and Ypred exchange as train_fused.cu
+// (eqs. 1-9; one launch for every batch of every epoch), but both large products
+// run on the tensor cores (tcgen05.mma kind::tf32: fp32 operands truncated to TF32, fp32
+// accumulate in TMEM):
+//   eq. 1  Z1 = X W1        per 256-row tile two chains M=128 (rows), N=32 (units of this CTA), K=32;
+//   eq. 8  dW1^T = dZ1^T X  one chain M=64 (32 units + padding), N=32 (inputs), K=256 rows, in TMEM
+//                           across the tiles of a batch.
 // Everything else stays fp32 on the CUDA cores.  Hidden 256 on a cluster of 8 CTAs only.
 //
-// Per tile and CTA (8 warps):
-//   TMA (cp.async.bulk.tensor, 128-byte swizzle) brings the X tile [256 x 32] one tile ahead;
-//   warp 0 issues the 8 MMAs (A = X tile, B = W1 slice kept in shared memory in operand layout);
-//   every thread owns ONE row: it reads its 32 pre-activations from TMEM (tcgen05.ld), applies
-//   eq. 2, stores H to shared memory, forms its partial of eq. 3 and pushes it to the 8 CTAs
-//   (st.async + mbarrier, as in train_fused.cu); after the exchange it computes dZ2 (eq. 5);
-//   the backward pass (eqs. 6-8) is the K-split FFMA2 loop of train_fused.cu reading H and dZ2
-//   from shared memory; per-warp partials, fixed-order cross-warp sum and eq. 9 as there, with
-//   the updated W1 written both to the fp32 master copy and to the MMA operand layout.
-// No W1 register file, hence no reload between steps.
+// Per tile and CTA (8 warps, a thread owns ONE row of the tile):
+//   TMA (cp.async.bulk.tensor, 128-byte swizzle) brings the X tile [256 x 32] one tile ahead; warp 0
+//   issues eq. 1 (A = X tile as delivered, B = W1^T slice in operand layout); while it runs every thread
+//   transposes its X row into the K-major B operand of eq. 8; then it reads its 32 pre-activations
+//   from TMEM, applies eq. 2, stores H, forms its partial of eq. 3 and pushes it to the 8 CTAs
+//   (st.async + mbarrier); after the exchange it computes dZ2 (eq. 5) and writes its row of
+//   dZ1 = dZ2 ReLU'(Z1) W2 (eq. 7) into the K-major A operand of eq. 8; warp 0 issues eq. 8 while all
+//   warps do eq. 6 (dW2) on the CUDA cores.  At the end of the batch the 32 threads that own the TMEM
+//   rows of dW1^T (one per hidden unit) apply eq. 9 to the fp32 master row they keep in registers and
+//   rewrite their row of the eq. 1 operand.  No W1 register reload, no CUDA-core backward loop.
+// All operands are K-major with the 128-byte swizzle (the conventions of eval_tf32.cu).
 #include <cuda.h>
 
 #include "common.cuh"
@@ -29,7 +33,7 @@ constexpr int kC = 8;             // cluster size
 constexpr int kBT = 256;          // rows per tile
 constexpr int kWarps = 8;
 constexpr int kThreads = kWarps * 32;
-constexpr int kRing = 3;          // X ring stages
+constexpr int kRing = 2;          // X ring stages (the operands of eq. 8 take the rest of shared memory)
 constexpr uint32_t kXBytes = kBT * kIn * 4;
 
 struct TcParams {
@@ -88,56 +92,61 @@ __device__ __forceinline__ bool elect_one() {
 __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
-// The gradient partials and the fp32 master copy keep hidden unit u in slot (u % 4) * 8 + u / 4, so that the
-// lanes of a sub-group (units 4*lu + j) store to consecutive 16-byte slots (no bank conflicts).
-__device__ __forceinline__ int unit_of(int sl) { return (sl & 7) * 4 + (sl >> 3); }
 // byte offset of the 16-byte chunk c of row r in a [rows][128 B] tile with the 128-byte swizzle
 __device__ __forceinline__ int swz(int r, int c) { return r * 128 + ((c ^ (r & 7)) << 4); }
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     constexpr int S = kS, BT = kBT, C = kC;
-    constexpr int LPS = 8, SPW = 4, RB = BT / SPW, ITER = RB / kWarps;   // backward mapping (train_fused.cu)
-    constexpr int IPS = kIn / SPW;                                        // inputs per sub-group
+    constexpr int NA = BT / 32;                                           // 32-row K atoms of the backward product
     extern __shared__ __align__(1024) unsigned char smem[];
-    unsigned char* Xs = smem;                                             // [kRing][32 KB] swizzled rows
-    unsigned char* Wop = Xs + kRing * kXBytes;                            // [S][128 B] B operand (K-major, swizzled)
-    unsigned char* Hs = Wop + S * 128;                                    // [BT][128 B] H = ReLU(Z1), swizzled rows
-    unsigned char* Ms = Hs + BT * 128;                                    // [BT][128 B] ReLU'(Z1) * W2 (eq. 7 factor), swizzled
-    float* part = reinterpret_cast<float*>(Ms + BT * 128);                // [kWarps][S*32]  layout [q][slot][4]
-    float* W1m = part + kWarps * S * kIn;                                 // [S*32] fp32 master, layout [q][slot][4]
-    float* ypp = W1m + S * kIn;                                           // [2][C][BT]
-    float* part2 = ypp + 2 * C * BT;                                      // [kWarps][S]
+    unsigned char* Xs = smem;                                             // [kRing][32 KB] X tiles, swizzled rows (A of eq. 1)
+    unsigned char* Wop = Xs + kRing * kXBytes;                            // [S][128 B] W1^T slice (B of eq. 1), K-major swizzled
+    unsigned char* At = Wop + S * 128;                                    // [NA][64][128 B] dZ1^T (A of eq. 8), rows 32-63 padding
+    unsigned char* Xt = At + NA * 64 * 128;                               // [NA][32][128 B] X^T (B of eq. 8)
+    unsigned char* Hs = Xt + NA * 32 * 128;                               // [BT][128 B] H = ReLU(Z1), swizzled rows (eq. 6)
+    float* ypp = reinterpret_cast<float*>(Hs + BT * 128);                 // [2][C][BT]
+    float* part2 = ypp + 2 * C * BT;                                      // [kWarps][S] dW2 partials
     float* W2s = part2 + kWarps * S;                                      // [S]
     float* Ds = W2s + S;                                                  // [BT] dZ2 of the tile
-    uint64_t* bars = reinterpret_cast<uint64_t*>(Ds + BT);                // full[3], empty[3], yp[2], mma
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kRing + 3);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Ds + BT);                // full[3], empty[3], yp[2], mma, mma2
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kRing + 4);
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kRing),
-                   bar_yp = smem_u32(bars + 2 * kRing), bar_mma = smem_u32(bars + 2 * kRing + 2);
+                   bar_yp = smem_u32(bars + 2 * kRing), bar_mma = smem_u32(bars + 2 * kRing + 2),
+                   bar_mma2 = smem_u32(bars + 2 * kRing + 3);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int lu = lane % LPS, s = lane / LPS;
     const uint32_t crank = cluster_ctarank();
     const int H = p.H;
+    // forward ownership: thread <-> tile row (TMEM lane rule: warp w reads lanes 32*(w%4)..)
+    const int frow = (warp >> 2) * 128 + (warp & 3) * 32 + lane;
+    // weight ownership: the M=64 accumulator of eq. 8 keeps unit u in TMEM lane (u/16)*32 + u%16, i.e. lanes
+    // 0-15 of warps 0 and 1: those 32 threads hold the fp32 master row W1[:, u] in registers for the whole run
+    const bool wowner = warp < 2 && lane < 16;
+    const int wu = warp * 16 + lane;                                      // owned hidden unit (if wowner)
+    float wrow[kIn];
+#pragma unroll
+    for (int i = 0; i < kIn; ++i) wrow[i] = wowner ? p.W1[(size_t)i * H + crank * S + wu] : 0.f;
+    auto store_wop = [&]() {                                              // B[n = u][k = i], eq. 1 operand
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            *reinterpret_cast<float4*>(Wop + swz(wu, c)) = make_float4(wrow[4 * c], wrow[4 * c + 1], wrow[4 * c + 2], wrow[4 * c + 3]);
+    };
 
     // ---- one-time setup ---------------------------------------------------------------------------
-    for (int f = tid; f < S * kIn; f += kThreads) {
-        const int q = f / (S * 4), rem = f % (S * 4), u = unit_of(rem >> 2), r = rem & 3, i = q * 4 + r;
-        const float w = p.W1[(size_t)i * H + crank * S + u];
-        W1m[f] = w;
-        *reinterpret_cast<float*>(Wop + swz(u, q) + r * 4) = w;           // B[n = u][k = i]
-    }
+    if (wowner) store_wop();
+    for (int f = tid; f < NA * 64 * 32; f += kThreads) reinterpret_cast<float*>(At)[f] = 0.f;   // padding rows stay 0
     if (tid < S) W2s[tid] = p.W2[crank * S + tid];
     if (tid == 0) {
         for (int b = 0; b < kRing; ++b) { mbar_init(bar_full + 8 * b, 1); mbar_init(bar_empty + 8 * b, kWarps); }
-        mbar_init(bar_yp, 1); mbar_init(bar_yp + 8, 1); mbar_init(bar_mma, 1);
+        mbar_init(bar_yp, 1); mbar_init(bar_yp + 8, 1); mbar_init(bar_mma, 1); mbar_init(bar_mma2, 1);
         fence_mbar_init();
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"(smem_u32(tmem_slot)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // Wop (generic writes) -> MMA (async proxy)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic writes -> MMA (async proxy)
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -158,21 +167,20 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     seq = 2 % p.nbi;
     if (tid == 0) issue_tile((long long)t_cur * p.B, 0);
 
-    // forward ownership: thread <-> tile row (TMEM lane rule: warp w reads lanes 32*(w%4)..)
-    const int frow = (warp >> 2) * 128 + (warp & 3) * 32 + lane;
-    const uint32_t taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (warp >> 2) * 32;
+    const uint32_t taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (warp >> 2) * 32;   // eq. 1 accumulators: columns 0-63
+    const uint32_t tdw = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + 64;                   // eq. 8 accumulator: columns 64-95
     float ycur = 0.f;
     {
         const long long r0 = (long long)t_cur * p.B;
         if (frow < min(BT, rows_of(t_cur))) ycur = __ldg(p.Y + r0 + frow);
     }
-    // Ypred exchange: peer CTA addresses
     const uint32_t ypp_a = smem_u32(ypp), yp_a = bar_yp;
-    const int rowl = warp * ITER;
-    float* mypart = part + warp * (S * kIn);
-
-    constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(S >> 3) << 17) |
-                               ((uint32_t)(128 >> 4) << 24);
+    // instruction descriptors: D=f32, A=B=tf32, both K-major; eq. 1: M=128, N=32; eq. 8: M=64, N=32
+    constexpr uint32_t idesc1 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(S >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+    constexpr uint32_t idesc8 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kIn >> 3) << 17) | ((uint32_t)(64 >> 4) << 24);
+    // position of (row r of the tile, column c) in the K-major operands of eq. 8: atom r/32, operand row c,
+    // k = r%32 inside the 128-byte swizzled row
+    const int ka = frow >> 5, kk = frow & 31;
     unsigned gt = 0;
     for (long long step = 0; step < total; ++step) {
         const int t_nn = (step + 2 < total) ? batch_index(step + 2, seq) : 0;
@@ -181,7 +189,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
         const int m = rows_of(t_cur);
         const int ntiles = (m + BT - 1) / BT;
         const float scale = t_cur == p.nbi - 1 ? p.scale_last : p.scale_full;   // eq. 5: 2 / m
-        float g2[4] = {0.f, 0.f, 0.f, 0.f};
+        float g2 = 0.f;                                        // dW2 partial: unit lane, rows 32*warp.. of every tile
 
         for (int j = 0; j < ntiles; ++j, ++gt) {
             const unsigned buf = gt & 1u, ph = (gt >> 1) & 1u;
@@ -202,8 +210,9 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
             float ynext = 0.f;
             if (frow < nrows) ynext = __ldg(p.Y + nr0 + frow);
 
-            // ---------------- forward: eq. 1 on the tensor cores ----------------
-            mbar_wait(bar_full + 8 * xst, xph);                // every warp reads X later (backward)
+            // ---------------- eq. 1 on the tensor cores ----------------
+            mbar_wait(bar_full + 8 * xst, xph);
+            const unsigned char* Xt_tile = Xs + xst * kXBytes;
             if (warp == 0) {
                 tc_fence_after();
                 if (elect_one()) {
@@ -213,15 +222,29 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                         const uint64_t adesc = smem_desc_sw128(smem_u32(Xs) + xst * kXBytes + a * 128 * 128);
 #pragma unroll
                         for (int k = 0; k < kIn / 8; ++k)
-                            mma_tf32(tmem_base + a * 32, adesc + 2 * k, bdesc + 2 * k, idesc, k > 0);
+                            mma_tf32(tmem_base + a * 32, adesc + 2 * k, bdesc + 2 * k, idesc1, k > 0);
                     }
                     tc_commit(bar_mma);
                 }
                 __syncwarp();
             }
+            // while the MMA runs: this thread's X row, transposed into the B operand of eq. 8
+            {
+                float xr[kIn];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    const float4 v = *reinterpret_cast<const float4*>(Xt_tile + swz(frow, c));
+                    xr[4 * c] = v.x; xr[4 * c + 1] = v.y; xr[4 * c + 2] = v.z; xr[4 * c + 3] = v.w;
+                }
+#pragma unroll
+                for (int i = 0; i < kIn; ++i)
+                    *reinterpret_cast<float*>(Xt + ka * (32 * 128) + swz(i, kk >> 2) + (kk & 3) * 4) = xr[i];
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp no longer reads the X tile
             mbar_wait(bar_mma, gt & 1u);
             tc_fence_after();
-            __syncthreads();                                   // every warp is done with H / dZ2 of the previous tile
+            float mk[kIn];                                     // ReLU'(z_u) w2_u of this row (eq. 7 factor, old W2)
             {
                 uint32_t z[32];
                 tmem_ld32(taddr, z);
@@ -235,8 +258,8 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                     h.x = fmaxf(__uint_as_float(z[4 * c]), 0.f);      h.y = fmaxf(__uint_as_float(z[4 * c + 1]), 0.f);   // eq. 2
                     h.z = fmaxf(__uint_as_float(z[4 * c + 2]), 0.f);  h.w = fmaxf(__uint_as_float(z[4 * c + 3]), 0.f);
                     *reinterpret_cast<float4*>(Hs + swz(frow, c)) = h;
-                    *reinterpret_cast<float4*>(Ms + swz(frow, c)) =                       // eq. 7: ReLU'(z) w2 (old W2)
-                        make_float4(h.x > 0.f ? w.x : 0.f, h.y > 0.f ? w.y : 0.f, h.z > 0.f ? w.z : 0.f, h.w > 0.f ? w.w : 0.f);
+                    mk[4 * c] = h.x > 0.f ? w.x : 0.f;     mk[4 * c + 1] = h.y > 0.f ? w.y : 0.f;
+                    mk[4 * c + 2] = h.z > 0.f ? w.z : 0.f; mk[4 * c + 3] = h.w > 0.f ? w.w : 0.f;
                     pr[c & 3] = fmaf(h.x, w.x, fmaf(h.y, w.y, fmaf(h.z, w.z, fmaf(h.w, w.w, pr[c & 3]))));   // eq. 3
                 }
                 const float pv = (pr[0] + pr[1]) + (pr[2] + pr[3]);
@@ -246,7 +269,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                     st_async_f32(mapa(ypp_a + (buf * (C * BT) + crank * BT + frow) * 4, d), pv, mapa(yp_a + 8 * buf, d));
                 }
             }
-            // ---------------- eq. 5 ----------------
+            // ---------------- eq. 5, eq. 7 ----------------
             mbar_wait(bar_yp + 8 * buf, ph);
             {
                 const float* ypt = ypp + buf * (C * BT);
@@ -257,98 +280,56 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 for (int o = 1; o < C; o <<= 1)
 #pragma unroll
                     for (int c = 0; c + o < C; c += 2 * o) ypc[c] += ypc[c + o];
-                Ds[frow] = frow < vt ? scale * (ypc[0] - ycur) : 0.f;
+                const float d = frow < vt ? scale * (ypc[0] - ycur) : 0.f;
+                Ds[frow] = d;
+#pragma unroll
+                for (int u = 0; u < S; ++u)                    // dZ1^T[u][row]: A operand of eq. 8
+                    *reinterpret_cast<float*>(At + ka * (64 * 128) + swz(u, kk >> 2) + (kk & 3) * 4) = d * mk[u];
             }
-            __syncthreads();                                   // H and dZ2 of the whole tile are in shared memory
-
-            // ---------------- backward: eqs. 6-8, K-split over the sub-groups ----------------
-            // lane (s, lu): units 4*lu..4*lu+3, inputs [IPS*s, IPS*(s+1)), rows of ALL sub-groups
-            const unsigned char* Xt = Xs + xst * kXBytes;
-            f32x2 acc[4][IPS / 2];
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // At, Xt (generic writes) -> MMA
+            __syncthreads();
+            // ---------------- eq. 8 on the tensor cores: dW1^T += dZ1^T X ----------------
+            if (warp == 0) {
+                tc_fence_after();
+                if (elect_one()) {
 #pragma unroll
-            for (int it = 0; it < ITER; ++it) {
+                    for (int a = 0; a < NA; ++a) {
+                        const uint64_t adesc = smem_desc_sw128(smem_u32(At) + a * (64 * 128));
+                        const uint64_t bdesc = smem_desc_sw128(smem_u32(Xt) + a * (32 * 128));
 #pragma unroll
-                for (int t = 0; t < SPW; ++t) {
-                    const int r = (s ^ t) * RB + rowl + it;                    // tile row
-                    const float d = Ds[r];
-                    const float4 mk = *reinterpret_cast<const float4*>(Ms + swz(r, lu));
-                    const float mm[4] = {mk.x, mk.y, mk.z, mk.w};
-                    if (t == 0) {                                              // eq. 6 (each row once per CTA)
-                        const float4 h = *reinterpret_cast<const float4*>(Hs + swz(r, lu));
-                        g2[0] = fmaf(h.x, d, g2[0]); g2[1] = fmaf(h.y, d, g2[1]);
-                        g2[2] = fmaf(h.z, d, g2[2]); g2[3] = fmaf(h.w, d, g2[3]);
+                        for (int k = 0; k < 4; ++k)
+                            mma_tf32(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
                     }
-                    f32x2 dd[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const float e = d * mm[u];                             // eq. 7
-                        dd[u] = pack2(e, e);
-                    }
-#pragma unroll
-                    for (int x = 0; x < IPS / 4; ++x) {                        // eq. 8
-                        const ulonglong2 xv = *reinterpret_cast<const ulonglong2*>(Xt + swz(r, (IPS / 4) * s + x));
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            if (it == 0 && t == 0) {
-                                acc[u][2 * x] = fmul2(xv.x, dd[u]);
-                                acc[u][2 * x + 1] = fmul2(xv.y, dd[u]);
-                            } else {
-                                ffma2(acc[u][2 * x], xv.x, dd[u]);
-                                ffma2(acc[u][2 * x + 1], xv.y, dd[u]);
-                            }
-                        }
-                    }
+                    tc_commit(bar_mma2);
                 }
+                __syncwarp();
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp is done with the X tile
+            // meanwhile eq. 6 on the CUDA cores: unit = lane, rows 32*warp .. 32*warp+31 of the tile
+#pragma unroll 8
+            for (int r = 0; r < 32; ++r) {
+                const int row = warp * 32 + r;
+                g2 = fmaf(*reinterpret_cast<const float*>(Hs + swz(row, lane >> 2) + (lane & 3) * 4), Ds[row], g2);
+            }
             ycur = ynext;
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-#pragma unroll
-                for (int x = 0; x < IPS / 4; ++x) {
-                    const int q = (IPS / 4) * s + x;
-                    ulonglong2* dst = reinterpret_cast<ulonglong2*>(mypart + (q * S + u * 8 + lu) * 4);   // slot_of(4*lu+u)
-                    f32x2 lo = acc[u][2 * x], hi = acc[u][2 * x + 1];
-                    if (j > 0) {                               // later tiles of a large batch
-                        const ulonglong2 old = *dst;
-                        lo = fadd2(lo, old.x); hi = fadd2(hi, old.y);
-                    }
-                    *dst = make_ulonglong2(lo, hi);
-                }
+            mbar_wait(bar_mma2, gt & 1u);                      // eq. 8 of this tile has read At / Xt
+            tc_fence_after();
+            __syncthreads();                                   // and every warp is done with Hs / Ds
         }
 
-        // ---------------- end of batch: reduce partial gradients, eq. 9 ----------------
+        // ---------------- end of batch: eq. 9 ----------------
+        part2[warp * S + lane] = g2;
+        if (warp < 2) {                                        // owners of the eq. 8 accumulator rows
+            uint32_t dw[32];
+            tmem_ld32(tdw, dw);
+            tmem_ld_wait();
+            tc_fence_before();
+            if (wowner) {
 #pragma unroll
-        for (int o = LPS; o < 32; o <<= 1)
-#pragma unroll
-            for (int u = 0; u < 4; ++u) g2[u] += __shfl_xor_sync(0xffffffffu, g2[u], o);
-        if (s == 0) {
-#pragma unroll
-            for (int u = 0; u < 4; ++u) part2[warp * S + 4 * lu + u] = g2[u];
+                for (int i = 0; i < kIn; ++i) wrow[i] = fmaf(-p.lr, __uint_as_float(dw[i]), wrow[i]);   // W - lr*dW
+                store_wop();
+            }
         }
         __syncthreads();
-        {
-            constexpr int NF = S * 8;                          // float4 slots of this CTA's dW1 (= kThreads)
-            const f32x2 nlr2 = pack2(-p.lr, -p.lr);
-            const int f = tid;
-            ulonglong2 v[kWarps];
-#pragma unroll
-            for (int w = 0; w < kWarps; ++w) v[w] = reinterpret_cast<const ulonglong2*>(part)[w * NF + f];
-#pragma unroll
-            for (int o = 1; o < kWarps; o <<= 1)               // fixed pairwise tree over warps
-#pragma unroll
-                for (int w = 0; w + o < kWarps; w += 2 * o) {
-                    v[w].x = fadd2(v[w].x, v[w + o].x);
-                    v[w].y = fadd2(v[w].y, v[w + o].y);
-                }
-            ulonglong2 wv = reinterpret_cast<ulonglong2*>(W1m)[f];
-            ffma2(wv.x, v[0].x, nlr2);                                         // eq. 9: W - lr*dW
-            ffma2(wv.y, v[0].y, nlr2);
-            reinterpret_cast<ulonglong2*>(W1m)[f] = wv;
-            const int q = f / S, u = unit_of(f % S);          // same float4 in the MMA operand layout
-            *reinterpret_cast<ulonglong2*>(Wop + swz(u, q)) = wv;
-        }
         if (tid < S) {
             float sum = part2[tid];
 #pragma unroll
@@ -362,16 +343,16 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     }
 
     // ---- write the trained slice back, free TMEM ---------------------------------------------------
-    for (int f = tid; f < S * kIn; f += kThreads) {
-        const int q = f / (S * 4), rem = f % (S * 4), u = unit_of(rem >> 2), i = q * 4 + (rem & 3);
-        p.W1[(size_t)i * H + crank * S + u] = W1m[f];
+    if (wowner) {
+#pragma unroll
+        for (int i = 0; i < kIn; ++i) p.W1[(size_t)i * H + crank * S + wu] = wrow[i];
     }
     if (tid < S) p.W2[crank * S + tid] = W2s[tid];
     tc_fence_before();
     __syncthreads();
     if (warp == 0) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" ::"r"(tmem_base) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem_base) : "memory");
     }
     cluster_sync_all();        // no CTA exits while peers may still push into its shared memory
 }
@@ -396,9 +377,8 @@ cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int bat
     if (p.total_steps == 0) return cudaSuccess;
     alignas(64) CUtensorMap tmap;
     if (!make_x_tensormap(&tmap, X, n, kBT)) return cudaErrorNotSupported;
-    const size_t smem = (size_t)kRing * kXBytes + kS * 128 + 2 * kBT * 128 +
-                        sizeof(float) * (kWarps * kS * kIn + kS * kIn + 2 * kC * kBT + kWarps * kS + kS + kBT) +
-                        8 * (2 * kRing + 3) + 16;
+    const size_t smem = (size_t)kRing * kXBytes + kS * 128 + (kBT / 32) * 64 * 128 + (kBT / 32) * 32 * 128 + kBT * 128 +
+                        sizeof(float) * (2 * kC * kBT + kWarps * kS + kS + kBT) + 8 * (2 * kRing + 4) + 16;
     cudaError_t err = cudaFuncSetAttribute(k_train_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     cudaLaunchConfig_t cfg = {};
