@@ -305,10 +305,14 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 __syncwarp();
             }
             // meanwhile eq. 6 on the CUDA cores: unit = lane, rows 32*warp .. 32*warp+31 of the tile
-#pragma unroll 8
-            for (int r = 0; r < 32; ++r) {
-                const int row = warp * 32 + r;
-                g2 = fmaf(*reinterpret_cast<const float*>(Hs + swz(row, lane >> 2) + (lane & 3) * 4), Ds[row], g2);
+            {
+                float gp[4] = {0.f, 0.f, 0.f, 0.f};            // four independent chains hide the LDS latency
+#pragma unroll
+                for (int r = 0; r < 32; ++r) {
+                    const int row = warp * 32 + r;
+                    gp[r & 3] = fmaf(*reinterpret_cast<const float*>(Hs + swz(row, lane >> 2) + (lane & 3) * 4), Ds[row], gp[r & 3]);
+                }
+                g2 += (gp[0] + gp[1]) + (gp[2] + gp[3]);
             }
             ycur = ynext;
             mbar_wait(bar_mma2, gt & 1u);                      // eq. 8 of this tile has read At / Xt
@@ -318,6 +322,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
         // ---------------- end of batch: eq. 9 ----------------
         part2[warp * S + lane] = g2;
+        __syncthreads();
         if (warp < 2) {                                        // owners of the eq. 8 accumulator rows
             uint32_t dw[32];
             tmem_ld32(tdw, dw);
@@ -328,13 +333,11 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 for (int i = 0; i < kIn; ++i) wrow[i] = fmaf(-p.lr, __uint_as_float(dw[i]), wrow[i]);   // W - lr*dW
                 store_wop();
             }
-        }
-        __syncthreads();
-        if (tid < S) {
-            float sum = part2[tid];
+        } else if (warp == 2) {                                // meanwhile eq. 9 for W2 (unit = lane)
+            float sum = part2[lane];
 #pragma unroll
-            for (int w = 1; w < kWarps; ++w) sum += part2[w * S + tid];
-            W2s[tid] -= p.lr * sum;                                            // eq. 9
+            for (int w = 1; w < kWarps; ++w) sum += part2[w * S + lane];
+            W2s[lane] -= p.lr * sum;
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // Wop -> next step's MMA
         __syncthreads();
