@@ -198,15 +198,17 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
             long long nr0 = 0; int nrows = 0;
             if (j + 1 < ntiles) { nr0 = r0 + (long long)(j + 1) * BT; nrows = min(BT, m - (j + 1) * BT); }
             else if (step + 1 < total) { nr0 = (long long)t_next * p.B; nrows = min(BT, rows_of(t_next)); }
-            if (tid == 0) {
-                mbar_arrive_expect_tx(bar_yp + 8 * buf, C * BT * 4);        // arm this tile's exchange
-                if (nrows > 0) {
-                    const unsigned g1 = gt + 1, nbuf = g1 % kRing;
-                    if (g1 >= kRing) mbar_wait(bar_empty + 8 * nbuf, ((g1 / kRing) - 1) & 1u);
-                    issue_tile(nr0, nbuf);
+            if (warp == 0) {                                   // converged warp, one elected lane (uniform-register forms)
+                if (elect_one()) {
+                    mbar_arrive_expect_tx(bar_yp + 8 * buf, C * BT * 4);    // arm this tile's exchange
+                    if (nrows > 0) {
+                        const unsigned g1 = gt + 1, nbuf = g1 % kRing;
+                        if (g1 >= kRing) mbar_wait(bar_empty + 8 * nbuf, ((g1 / kRing) - 1) & 1u);
+                        issue_tile(nr0, nbuf);
+                    }
                 }
+                __syncwarp();
             }
-            __syncwarp();
             float ynext = 0.f;
             if (frow < nrows) ynext = __ldg(p.Y + nr0 + frow);
 
