@@ -72,15 +72,6 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// one lane of a converged warp (the MMA / TMA issue must not sit behind a divergent branch: UTCHMMA
-// and UTMALDG take uniform registers, and ptxas wraps them in per-lane loops otherwise)
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred = 0;
-    asm volatile(
-        "{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}"
-        : "=r"(pred));
-    return pred != 0;
-}
 
 // K-major, 128-byte-swizzled operand descriptor (8-row x 128-byte atoms, 1024 bytes apart)
 __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
