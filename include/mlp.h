@@ -49,7 +49,7 @@ enum {
                               /* eval:     streaming fp32 kernel (FFMA)                          */
     MLP_VARIANT_UNFUSED = 1,  /* training: one kernel per equation, launched per step (baseline) */
     MLP_VARIANT_TF32 = 2,     /* eval and training: eq. 1 on the tensor cores (tcgen05, TF32 operands, fp32
-                                 accumulate); separately reported, own tolerance; training: hidden 256 only */
+                                 accumulate); separately reported, own tolerance; training: hidden <= 256 */
     MLP_VARIANT_PRIOR_NAIVE = 3, /* training: the paper's baseline, naive 16x16 matmul kernels; comparison only */
     MLP_VARIANT_PRIOR_TILED = 4  /* training: the paper's optimised strategy, tiled + transposed + fused ReLU; comparison only */
 };

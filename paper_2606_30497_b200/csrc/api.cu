@@ -148,7 +148,7 @@ int train_impl(const float* X, const float* Y, int64_t n, int batch, float lr, i
     }
     if (variant == MLP_VARIANT_TF32) {
         if (!train_tf32_supported(g.hidden))
-            return fail(MLP_ERR_UNSUPPORTED, "TF32 training variant needs hidden 256 (got %d)", g.hidden);
+            return fail(MLP_ERR_UNSUPPORTED, "TF32 training variant supports hidden 32..256 (got %d)", g.hidden);
         cudaError_t e = launch_train_tf32(X, Y, n, batch, lr, epochs, W1, W2, order, g.hidden, stream, &g.launches);
         if (e != cudaSuccess) return cuda_fail(e, "launch_train_tf32");
         return MLP_OK;

@@ -7,7 +7,9 @@
 //   eq. 1  Z1 = X W1        per 256-row tile two chains M=128 (rows), N=32 (units of this CTA), K=32;
 //   eq. 8  dW1^T = dZ1^T X  one chain M=64 (32 units + padding), N=32 (inputs), K=256 rows, in TMEM
 //                           across the tiles of a batch.
-// Everything else stays fp32 on the CUDA cores.  Hidden 256 on a cluster of 8 CTAs only.
+// Everything else stays fp32 on the CUDA cores.  32 hidden units per CTA: hidden 32..256 on a
+// cluster of hidden/32 CTAs (the exchange buffers of a 16-CTA cluster no longer fit beside the
+// operands of eq. 8 in shared memory; hidden 1024 would need 32 CTAs per cluster).
 //
 // Per tile and CTA (8 warps, a thread owns ONE row of the tile):
 //   TMA (cp.async.bulk.tensor, 128-byte swizzle) brings the X tile [256 x 32] one tile ahead; warp 0
@@ -29,7 +31,7 @@ namespace mlp {
 namespace {
 
 constexpr int kS = 32;            // hidden units per CTA
-constexpr int kC = 8;             // cluster size
+// cluster size C = hidden / 32 is a template parameter (1, 2, 4 or 8)
 constexpr int kBT = 256;          // rows per tile
 constexpr int kWarps = 8;
 constexpr int kThreads = kWarps * 32;
@@ -90,9 +92,10 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
 // byte offset of the 16-byte chunk c of row r in a [rows][128 B] tile with the 128-byte swizzle
 __device__ __forceinline__ int swz(int r, int c) { return r * 128 + ((c ^ (r & 7)) << 4); }
 
+template <int C>
 __global__ void __launch_bounds__(kThreads, 1)
 k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
-    constexpr int S = kS, BT = kBT, C = kC;
+    constexpr int S = kS, BT = kBT;
     constexpr int NA = BT / 32;                                           // 32-row K atoms of the backward product
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* Xs = smem;                                             // [kRing][32 KB] X tiles, swizzled rows (A of eq. 1)
@@ -359,12 +362,15 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
 }  // namespace
 
-bool train_tf32_supported(int hidden) { return hidden == kS * kC; }
+bool train_tf32_supported(int hidden) {
+    return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256;
+}
 
 cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
                               float* W1, float* W2, const int32_t* order, int hidden,
                               cudaStream_t stream, int64_t* launches) {
-    if (hidden != kS * kC || n > 0x7fffffffLL - kBT) return cudaErrorInvalidValue;
+    if (!train_tf32_supported(hidden) || n > 0x7fffffffLL - kBT) return cudaErrorInvalidValue;
+    const int C = hidden / kS;
     TcParams p;
     p.Y = Y; p.n = n; p.B = batch; p.lr = lr;
     const long long nb = (n + batch - 1) / batch;
@@ -378,22 +384,36 @@ cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int bat
     alignas(64) CUtensorMap tmap;
     if (!make_x_tensormap(&tmap, X, n, kBT)) return cudaErrorNotSupported;
     const size_t smem = (size_t)kRing * kXBytes + kS * 128 + (kBT / 32) * 64 * 128 + (kBT / 32) * 32 * 128 + kBT * 128 +
-                        sizeof(float) * (2 * kC * kBT + kWarps * kS + kS + kBT) + 8 * (2 * kRing + 4) + 16;
-    cudaError_t err = cudaFuncSetAttribute(k_train_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(kC);
-    cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = kC;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    err = cudaLaunchKernelEx(&cfg, k_train_tf32, tmap, p);
+                        sizeof(float) * (2 * C * kBT + kWarps * kS + kS + kBT) + 8 * (2 * kRing + 4) + 16;
+    auto launch = [&](auto kern) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        if (C > 8) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (e != cudaSuccess) return e;
+        }
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(C);
+        cfg.blockDim = dim3(kThreads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = C;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, kern, tmap, p);
+    };
+    cudaError_t err;
+    switch (C) {
+        case 1: err = launch(k_train_tf32<1>); break;
+        case 2: err = launch(k_train_tf32<2>); break;
+        case 4: err = launch(k_train_tf32<4>); break;
+        case 8: err = launch(k_train_tf32<8>); break;
+        default: return cudaErrorInvalidValue;
+    }
     if (err == cudaSuccess) ++*launches;
     return err;
 }

@@ -161,6 +161,25 @@ def test_train_tf32_variant_batches_and_ragged(batch, n):
     assert np.array_equal(g1, h1) and np.array_equal(g2, h2)              # deterministic
 
 
+@pytest.mark.parametrize("hidden", [32, 64, 128])
+def test_train_tf32_variant_hidden_sweep(hidden):
+    n = 4096
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(2, 32, hidden)
+    order = datagen.make_order(n, 256, 2, True)
+    o1, o2 = O.train(X, Y, W1, W2, 256, LR, 2, order=order)
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 2, order=order, variant=B.VARIANT_TF32)
+    assert nerr(g1, o1) <= 2e-3 and nerr(g2, o2) <= 2e-3, (hidden, nerr(g1, o1), nerr(g2, o2))
+
+
+def test_train_tf32_variant_unsupported_hidden():
+    X, Y = datagen.make_dataset(512, 0.1)
+    for hidden in (512, 1024):
+        W1, W2 = O.init_weights(2, 32, hidden)
+        with pytest.raises(B.MlpError):
+            gpu_train(X, Y, W1, W2, 256, LR, 1, variant=B.VARIANT_TF32)
+
+
 # ------------------------------------------------------------------ config 2 (shuffled batch order)
 def test_config2_epoch_and_final_loss():
     c = datagen.CONFIGS["config2"]
