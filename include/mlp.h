@@ -21,8 +21,13 @@
  *   - Functions returning int return MLP_OK (0) or a positive mlp_status; nothing throws or
  *     calls exit().  Errors detected before launch leave W1/W2 untouched.  mlp_last_error()
  *     describes the most recent failure on the calling thread.
- *   - One model descriptor per process (set by mlp_init); calls on different streams with
- *     different buffers may overlap.
+ *   - Concurrency: one model descriptor per process (set by mlp_init).  Calls on different streams
+ *     with different caller buffers may overlap on the device: every eval launch takes its own
+ *     workspace (per-CTA partial sums, ticket, result) from a library-owned pool of 32 slots, a slot
+ *     being reused only after the launch that last used it has completed (the later stream is made
+ *     to wait otherwise), and every fused training launch writes its statistics to its own slot
+ *     (64 slots).  mlp_eval_loss_ws takes a caller-owned workspace instead.  The entry points
+ *     themselves are serialised by a mutex (enqueueing is cheap; the kernels run asynchronously).
  *   - There is no CPU fallback: without a CUDA device every compute entry returns MLP_ERR_CUDA.
  */
 #ifndef PAPER_2606_30497_MLP_H
@@ -51,7 +56,11 @@ enum {
     MLP_VARIANT_TF32 = 2,     /* eval and training: eq. 1 on the tensor cores (tcgen05, TF32 operands, fp32
                                  accumulate); separately reported, own tolerance; training: hidden <= 256 */
     MLP_VARIANT_PRIOR_NAIVE = 3, /* training: the paper's baseline, naive 16x16 matmul kernels; comparison only */
-    MLP_VARIANT_PRIOR_TILED = 4  /* training: the paper's optimised strategy, tiled + transposed + fused ReLU; comparison only */
+    MLP_VARIANT_PRIOR_TILED = 4, /* training: the paper's optimised strategy, tiled + transposed + fused ReLU; comparison only */
+    MLP_VARIANT_BF16 = 5,     /* eval and training: as MLP_VARIANT_TF32 with BF16 operands (converted in the kernel, round to
+                                 nearest even; tcgen05.mma kind::f16, fp32 accumulate); separately reported, own tolerance */
+    MLP_VARIANT_TF32X3 = 6    /* eval only: eq. 1 as three TF32 products (X = Xh + Xl, W = Wh + Wl; Xh Wh + Xh Wl + Xl Wh),
+                                 fp32-faithful to ~1e-6; separately reported */
 };
 
 /*
@@ -89,7 +98,10 @@ int mlp_train(const float* X, const float* Y, int64_t n, int batch, float lr, in
  * mlp_train_ex -- as mlp_train, plus
  *   batch_order: NULL, or device int32 [epochs * nb], nb = ceil(n/batch): step e*nb+k trains on
  *                batch index batch_order[e*nb+k] (BASELINE.json configs 2-5: "batch order a
- *                per-epoch permutation").  Entries must lie in [0, nb); not validated on device.
+ *                per-epoch permutation").  Entries must lie in [0, nb).  The device kernels clamp an
+ *                out-of-range entry into [0, nb) (no out-of-bounds access) and count it: see
+ *                mlp_train_order_errors().  The per-equation variants and the host entry points
+ *                validate the table on the host and return MLP_ERR_BAD_ARG before any work.
  *   variant:     MLP_VARIANT_FUSED, MLP_VARIANT_UNFUSED, MLP_VARIANT_PRIOR_NAIVE, MLP_VARIANT_PRIOR_TILED, or
  *                MLP_VARIANT_TF32 (stated tolerance vs the exact path: weights within 5e-5 after one step,
  *                2e-3 after one epoch, loss within 1 %).
@@ -101,7 +113,8 @@ int mlp_train_ex(const float* X, const float* Y, int64_t n, int batch, float lr,
  * mlp_train_rows -- mini-batch SGD with SAMPLE-level shuffling (the other reading of "batch order",
  * DESIGN.md reading 5; the paper is silent on shuffling): in epoch e, batch k is
  * rows row_order[e*n + k*batch .. e*n + min(n, (k+1)*batch)) of X/Y.
- *   row_order: DEVICE int32 [epochs*n], each epoch a permutation of 0..n-1 (not validated).
+ *   row_order: DEVICE int32 [epochs*n], each epoch a permutation of 0..n-1 (entries outside [0, n) are
+ *              clamped and counted, see mlp_train_order_errors(); duplicates are not detected).
  * Per epoch the rows are gathered into library-owned scratch (one pass at HBM speed) and the fused
  * kernel runs the epoch on the gathered copy: two launches per epoch.  Same arithmetic, same
  * error behaviour and asynchrony as mlp_train; the scratch (n*132 bytes) is freed by mlp_shutdown.
@@ -127,13 +140,37 @@ int mlp_eval_loss_async(const float* X, const float* Y, int64_t n, const float* 
                         const float* W2, double* d_out, int variant, void* stream);
 
 /*
+ * mlp_eval_loss_ws -- mlp_eval_loss_async with a CALLER-owned workspace instead of a pool slot:
+ * `workspace` is a device buffer of at least mlp_eval_workspace_bytes() bytes, 8-byte aligned, whose
+ * first use must find it zero-filled (the kernel leaves it reusable); launches that may run
+ * concurrently need distinct workspaces.  mlp_eval_workspace_bytes() returns 0 without a CUDA device.
+ */
+size_t mlp_eval_workspace_bytes(void);
+int mlp_eval_loss_ws(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+                     double* d_out, int variant, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Host-buffer entry points (end-to-end path): copy X/Y (and weights / order) from HOST memory
  * to library-owned device buffers, run the same kernels, copy the result back, synchronise.
- * W1_host/W2_host are read and overwritten with the trained weights.  order_host may be NULL.
+ * W1_host/W2_host are read and overwritten with the trained weights.  order_host may be NULL; if
+ * given, every entry is validated on the host first (MLP_ERR_BAD_ARG, nothing copied or launched).
+ *   mlp_train_host      the whole job in one training launch.
+ *   mlp_fit_host        BASELINE.json configs[2]: training with "a full-dataset eval-loss pass after
+ *                       each epoch" (eq. 4): one training launch and one eval launch (eval_variant) per
+ *                       epoch, all asynchronous behind one copy of the dataset; epoch_loss_host [epochs]
+ *                       receives the losses (NULL: no evaluation, identical to mlp_train_host).
+ *   mlp_eval_loss_host  X/Y are copied in 32 MiB chunks on a second stream and the eval kernel of a
+ *                       chunk starts as soon as the chunk has landed (copy and compute overlap; the
+ *                       pass is PCIe-bound).  The dataset loss is the row-weighted mean of the per-chunk
+ *                       means, formed in chunk order (deterministic); n <= 262,144 rows is one chunk and
+ *                       returns exactly what mlp_eval_loss returns.
  */
 int mlp_train_host(const float* X_host, const float* Y_host, int64_t n, int batch, float lr,
                    int epochs, float* W1_host, float* W2_host, const int32_t* order_host,
                    int variant);
+int mlp_fit_host(const float* X_host, const float* Y_host, int64_t n, int batch, float lr, int epochs,
+                 float* W1_host, float* W2_host, const int32_t* order_host, int variant,
+                 int eval_variant, double* epoch_loss_host);
 double mlp_eval_loss_host(const float* X_host, const float* Y_host, int64_t n,
                           const float* W1_host, const float* W2_host, int variant);
 
@@ -143,14 +180,23 @@ double mlp_eval_loss_host(const float* X_host, const float* Y_host, int64_t n,
  * {16, 32, 64} and cluster in {1, 2, 4, 8, 16}.  Returns MLP_ERR_UNSUPPORTED otherwise.
  */
 int mlp_set_cluster(int cluster);
-int mlp_get_cluster(void);          /* the cluster size the next mlp_train would use */
+int mlp_get_cluster(void);          /* the cluster size the next mlp_train would use at batch 256 */
+int mlp_get_cluster_for(int batch); /* ... at the given batch size (the automatic choice depends on it) */
 
 /*
- * Statistics of the most recent fused mlp_train* call that has completed (call after
- * synchronising its stream): out[0] = SM clock cycles spent in the kernel (clock64 delta of
- * CTA 0), out[1] = nanoseconds (globaltimer delta), out[2] = SGD steps, out[3] = cluster size.
+ * Statistics of the most recently ISSUED fused mlp_train* launch (call after synchronising its
+ * stream; concurrent launches each have their own slot, so they do not disturb each other):
+ * out[0] = SM clock cycles spent in the kernel (clock64 delta of CTA 0), out[1] = nanoseconds
+ * (globaltimer delta), out[2] = SGD steps, out[3] = cluster size.
  */
 int mlp_get_train_stats(double out[4]);
+
+/*
+ * Number of batch_order / row_order entries of that launch (for mlp_train_rows: of that call) that
+ * were outside their valid range and were clamped by the device kernels; 0 for a valid table,
+ * -1 on a CUDA error.  Call after synchronising the stream.
+ */
+int64_t mlp_train_order_errors(void);
 
 /* Number of kernels this library has launched since load (all entry points). */
 int64_t mlp_launch_count(void);

@@ -20,12 +20,15 @@ VARIANT_UNFUSED = 1
 VARIANT_TF32 = 2
 VARIANT_PRIOR_NAIVE = 3
 VARIANT_PRIOR_TILED = 4
+VARIANT_BF16 = 5
+VARIANT_TF32X3 = 6
 
 EXPORTS = [
     "mlp_init", "mlp_init_weights", "mlp_train", "mlp_train_ex", "mlp_eval_loss",
-    "mlp_eval_loss_async", "mlp_train_host", "mlp_eval_loss_host", "mlp_set_cluster",
-    "mlp_train_rows", "mlp_get_cluster", "mlp_get_train_stats", "mlp_launch_count", "mlp_last_error",
-    "mlp_version", "mlp_shutdown",
+    "mlp_eval_loss_async", "mlp_eval_loss_ws", "mlp_eval_workspace_bytes", "mlp_train_host", "mlp_fit_host",
+    "mlp_eval_loss_host", "mlp_set_cluster", "mlp_train_rows", "mlp_get_cluster", "mlp_get_cluster_for",
+    "mlp_get_train_stats", "mlp_train_order_errors", "mlp_launch_count", "mlp_last_error", "mlp_version",
+    "mlp_shutdown",
 ]
 
 
@@ -57,8 +60,15 @@ def lib():
     L.mlp_eval_loss.argtypes = [vp, vp, i64, vp, vp, vp]; L.mlp_eval_loss.restype = f64
     L.mlp_eval_loss_async.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp]
     L.mlp_eval_loss_async.restype = i32
+    L.mlp_eval_loss_ws.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp, C.c_size_t, vp]
+    L.mlp_eval_loss_ws.restype = i32
+    L.mlp_eval_workspace_bytes.argtypes = []; L.mlp_eval_workspace_bytes.restype = C.c_size_t
     L.mlp_train_host.argtypes = [vp, vp, i64, i32, f32, i32, vp, vp, vp, i32]
     L.mlp_train_host.restype = i32
+    L.mlp_fit_host.argtypes = [vp, vp, i64, i32, f32, i32, vp, vp, vp, i32, i32, vp]
+    L.mlp_fit_host.restype = i32
+    L.mlp_get_cluster_for.argtypes = [i32]; L.mlp_get_cluster_for.restype = i32
+    L.mlp_train_order_errors.argtypes = []; L.mlp_train_order_errors.restype = i64
     L.mlp_eval_loss_host.argtypes = [vp, vp, i64, vp, vp, i32]; L.mlp_eval_loss_host.restype = f64
     L.mlp_set_cluster.argtypes = [i32]; L.mlp_set_cluster.restype = i32
     L.mlp_get_cluster.argtypes = []; L.mlp_get_cluster.restype = i32
@@ -136,6 +146,20 @@ def mlp_eval_loss_async(X, Y, n, W1, W2, d_out, variant=VARIANT_FUSED, stream=No
                                      _dptr(d_out, "float64", "d_out"), int(variant), _stream(stream)))
 
 
+def mlp_eval_workspace_bytes() -> int:
+    return int(lib().mlp_eval_workspace_bytes())
+
+
+def mlp_eval_loss_ws(X, Y, n, W1, W2, d_out, variant, workspace, stream=None) -> None:
+    if not (workspace.is_cuda and workspace.is_contiguous()):
+        raise TypeError("workspace: need a contiguous CUDA tensor")
+    _check(lib().mlp_eval_loss_ws(_dptr(X, "float32", "X"), _dptr(Y, "float32", "Y"), int(n),
+                                  _dptr(W1, "float32", "W1"), _dptr(W2, "float32", "W2"),
+                                  _dptr(d_out, "float64", "d_out"), int(variant),
+                                  C.c_void_p(workspace.data_ptr()), workspace.numel() * workspace.element_size(),
+                                  _stream(stream)))
+
+
 def _hptr(a, dtype, what):
     """Host pointer of a C-contiguous numpy array or CPU torch tensor (pinned or not)."""
     if isinstance(a, np.ndarray):
@@ -154,6 +178,15 @@ def mlp_train_host(X, Y, n, batch, lr, epochs, W1, W2, order=None, variant=VARIA
                                 _hptr(W2, np.float32, "W2"), op, int(variant)))
 
 
+def mlp_fit_host(X, Y, n, batch, lr, epochs, W1, W2, order=None, variant=VARIANT_FUSED,
+                 eval_variant=VARIANT_FUSED, epoch_loss=None) -> None:
+    op = _hptr(order, np.int32, "order") if order is not None else None
+    lp = _hptr(epoch_loss, np.float64, "epoch_loss") if epoch_loss is not None else None
+    _check(lib().mlp_fit_host(_hptr(X, np.float32, "X"), _hptr(Y, np.float32, "Y"), int(n),
+                              int(batch), float(lr), int(epochs), _hptr(W1, np.float32, "W1"),
+                              _hptr(W2, np.float32, "W2"), op, int(variant), int(eval_variant), lp))
+
+
 def mlp_eval_loss_host(X, Y, n, W1, W2, variant=VARIANT_FUSED) -> float:
     v = lib().mlp_eval_loss_host(_hptr(X, np.float32, "X"), _hptr(Y, np.float32, "Y"), int(n),
                                  _hptr(W1, np.float32, "W1"), _hptr(W2, np.float32, "W2"), int(variant))
@@ -166,8 +199,12 @@ def mlp_set_cluster(cluster: int) -> None:
     _check(lib().mlp_set_cluster(int(cluster)))
 
 
-def mlp_get_cluster() -> int:
-    return int(lib().mlp_get_cluster())
+def mlp_get_cluster(batch=None) -> int:
+    return int(lib().mlp_get_cluster() if batch is None else lib().mlp_get_cluster_for(int(batch)))
+
+
+def mlp_train_order_errors() -> int:
+    return int(lib().mlp_train_order_errors())
 
 
 def mlp_get_train_stats():

@@ -12,8 +12,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmlp_b200.so")
-SOURCES = ["api.cu", "train_fused.cu", "eval_fp32.cu", "eval_tf32.cu", "train_tf32.cu", "unfused.cu", "prior_art.cu"]
-HEADERS = ["common.cuh", "internal.h", os.path.join("..", "..", "include", "mlp.h")]
+SOURCES = ["api.cu", "train_fused.cu", "eval_fp32.cu", "eval_tc.cu", "train_tc.cu", "unfused.cu", "prior_art.cu"]
+HEADERS = ["common.cuh", "tc_common.cuh", "internal.h", os.path.join("..", "..", "include", "mlp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

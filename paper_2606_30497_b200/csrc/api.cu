@@ -1,6 +1,8 @@
 // api.cu -- the C-ABI of libmlp_b200 (include/mlp.h): argument validation, library state,
 // lazily created device scratch, host-buffer (end-to-end) entry points.  No arithmetic of the
 // method lives here; every step of the path runs in the kernels of the other translation units.
+// (The only sums formed on the host are the fixed-order combination of per-chunk mean losses in
+// mlp_eval_loss_host, which is bookkeeping of eq. 4's 1/n, see there.)
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -15,22 +17,36 @@ namespace {
 
 using namespace mlp;
 
+constexpr int kEvalSlots = 32;     // eval launches in flight that never share a workspace
+constexpr int kStatSlots = 64;     // fused training launches in flight with their own statistics
+constexpr int kHostChunks = 64;    // at most this many chunks in the pipelined copy of mlp_eval_loss_host
+constexpr int64_t kChunkRows = 1 << 18;   // 32 MiB of X per chunk
+
 struct State {
     bool init = false;
     uint64_t seed = 0;
     int in = 0, hidden = 0, out = 0;
     int cluster = 0;                  // 0 = automatic
     int num_sms = 0;
-    // scratch
-    double* eval_partials = nullptr;  int eval_partials_cap = 0;
-    double* eval_out = nullptr;       // device double for the synchronous entry
-    unsigned long long* stats = nullptr;
+    // Every eval launch gets its own workspace slot (per-CTA partials, ticket, result) and every
+    // fused training launch its own statistics slot, so calls on different streams never share
+    // library-owned device memory (include/mlp.h, "Concurrency").
+    double* eval_pool = nullptr;      // [kEvalSlots][eval_stride]
+    size_t eval_stride = 0;           // doubles per slot: num_sms partials + ticket + result
+    cudaEvent_t eval_done[kEvalSlots] = {};
+    bool eval_zeroed[kEvalSlots] = {};
+    unsigned eval_next = 0;
+    unsigned long long* stats = nullptr;   // [kStatSlots][kStatWords]
+    unsigned stats_next = 0;
+    int stats_latest = -1;
     UnfusedScratch unf = {};          int unf_batch = 0, unf_hidden = 0;
     float *priorXT = nullptr, *priorHT = nullptr;   // transposes of the paper's tiled strategy
     float *shufX = nullptr, *shufY = nullptr; size_t shufX_cap = 0, shufY_cap = 0;   // mlp_train_rows
     float *hX = nullptr, *hY = nullptr, *hW1 = nullptr, *hW2 = nullptr; int32_t* hOrder = nullptr;
-    size_t hX_cap = 0, hY_cap = 0, hW_cap = 0, hOrder_cap = 0;
-    cudaStream_t host_stream = nullptr;
+    double* hLoss = nullptr;
+    size_t hX_cap = 0, hY_cap = 0, hW_cap = 0, hOrder_cap = 0, hLoss_cap = 0;
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
+    cudaEvent_t chunk_ev[kHostChunks] = {};
     int64_t launches = 0;
 };
 State g;
@@ -71,16 +87,63 @@ int grow(T** p, size_t* cap, size_t need) {
     return MLP_OK;
 }
 
-int ensure_eval_scratch(int grid) {
-    if (g.eval_partials_cap < grid + 1) {
-        if (g.eval_partials) CK(cudaFree(g.eval_partials));
-        g.eval_partials = nullptr; g.eval_partials_cap = 0;
-        CK(cudaMalloc(reinterpret_cast<void**>(&g.eval_partials), sizeof(double) * (grid + 1)));
-        CK(cudaMemset(g.eval_partials, 0, sizeof(double) * (grid + 1)));   // ticket counter = 0
-        g.eval_partials_cap = grid + 1;
+// A workspace of the eval kernels: `grid` per-CTA partial sums (double), the last-block ticket, and
+// one double for the result of the synchronous entry points.
+struct EvalWs {
+    double* partials;
+    unsigned int* ticket;
+    double* result;
+    int slot;          // pool slot, or -1 for a caller-supplied workspace
+};
+
+size_t eval_ws_doubles() { return (size_t)g.num_sms + 2; }
+
+// Takes the next slot of the pool for a launch on `stream`.  A slot is reused only after the launch
+// that last used it has completed: if it has not, `stream` is made to wait for it.  The ticket is
+// zeroed on first use, on the launching stream, and re-zeroed by the kernel's last block.
+int acquire_eval_slot(cudaStream_t stream, EvalWs* ws) {
+    int rc = ensure_device();
+    if (rc) return rc;
+    if (!g.eval_pool) {
+        g.eval_stride = (eval_ws_doubles() + 15) / 16 * 16;       // 128-byte slots
+        CK(cudaMalloc(reinterpret_cast<void**>(&g.eval_pool), sizeof(double) * g.eval_stride * kEvalSlots));
+        for (int i = 0; i < kEvalSlots; ++i) {
+            CK(cudaEventCreateWithFlags(&g.eval_done[i], cudaEventDisableTiming));
+            g.eval_zeroed[i] = false;
+        }
     }
-    if (!g.eval_out) CK(cudaMalloc(reinterpret_cast<void**>(&g.eval_out), sizeof(double)));
+    const int slot = (int)(g.eval_next++ % kEvalSlots);
+    double* base = g.eval_pool + (size_t)slot * g.eval_stride;
+    if (!g.eval_zeroed[slot]) {
+        CK(cudaMemsetAsync(base, 0, sizeof(double) * g.eval_stride, stream));
+        g.eval_zeroed[slot] = true;
+    } else if (cudaEventQuery(g.eval_done[slot]) != cudaSuccess) {
+        (void)cudaGetLastError();                                  // cudaErrorNotReady is not sticky
+        CK(cudaStreamWaitEvent(stream, g.eval_done[slot], 0));
+    }
+    ws->partials = base;
+    ws->ticket = reinterpret_cast<unsigned int*>(base + g.num_sms);
+    ws->result = base + g.num_sms + 1;
+    ws->slot = slot;
     return MLP_OK;
+}
+
+int release_eval_slot(const EvalWs& ws, cudaStream_t stream) {
+    if (ws.slot >= 0) CK(cudaEventRecord(g.eval_done[ws.slot], stream));
+    return MLP_OK;
+}
+
+unsigned long long* acquire_stats_slot() {
+    if (!g.stats) {
+        if (cudaMalloc(reinterpret_cast<void**>(&g.stats), sizeof(unsigned long long) * kStatWords * kStatSlots) != cudaSuccess ||
+            cudaMemset(g.stats, 0, sizeof(unsigned long long) * kStatWords * kStatSlots) != cudaSuccess) {
+            g.stats = nullptr;
+            return nullptr;
+        }
+    }
+    const int slot = (int)(g.stats_next++ % kStatSlots);
+    g.stats_latest = slot;
+    return g.stats + (size_t)slot * kStatWords;
 }
 
 int ensure_unfused(int batch, int hidden) {
@@ -102,8 +165,13 @@ int ensure_unfused(int batch, int hidden) {
     return MLP_OK;
 }
 
-int effective_cluster() {
-    return g.cluster ? g.cluster : fused_default_cluster(g.hidden);
+int effective_cluster(int batch) {
+    return g.cluster ? g.cluster : fused_default_cluster(g.hidden, batch);
+}
+
+bool known_train_variant(int v) {
+    return v == MLP_VARIANT_FUSED || v == MLP_VARIANT_UNFUSED || v == MLP_VARIANT_TF32 || v == MLP_VARIANT_BF16 ||
+           v == MLP_VARIANT_PRIOR_NAIVE || v == MLP_VARIANT_PRIOR_TILED;
 }
 
 int check_train_args(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
@@ -114,8 +182,7 @@ int check_train_args(const float* X, const float* Y, int64_t n, int batch, float
     if (batch < 1) return fail(MLP_ERR_BAD_ARG, "batch must be >= 1 (got %d)", batch);
     if (epochs < 0) return fail(MLP_ERR_BAD_ARG, "epochs must be >= 0 (got %d)", epochs);
     if (!std::isfinite(lr)) return fail(MLP_ERR_BAD_ARG, "lr must be finite");
-    if (variant != MLP_VARIANT_FUSED && variant != MLP_VARIANT_UNFUSED && variant != MLP_VARIANT_TF32 &&
-        variant != MLP_VARIANT_PRIOR_NAIVE && variant != MLP_VARIANT_PRIOR_TILED)
+    if (!known_train_variant(variant))
         return fail(MLP_ERR_UNSUPPORTED, "training variant %d is not supported", variant);
     if (((uintptr_t)X & 15) || ((uintptr_t)W1 & 15))
         return fail(MLP_ERR_ALIGN, "X and W1 must be 16-byte aligned");
@@ -124,36 +191,55 @@ int check_train_args(const float* X, const float* Y, int64_t n, int batch, float
     const int64_t nb = (n + batch - 1) / batch;
     if (nb > 0x7fffffffLL) return fail(MLP_ERR_BAD_ARG, "too many batches per epoch (batch indices are int32)");
     if (nb * (int64_t)epochs > (int64_t)1 << 40) return fail(MLP_ERR_BAD_ARG, "too many steps");
+    const bool per_equation = variant == MLP_VARIANT_UNFUSED || variant == MLP_VARIANT_PRIOR_NAIVE ||
+                              variant == MLP_VARIANT_PRIOR_TILED;
+    const int64_t rows = batch < n ? batch : n;
+    if (per_equation && rows * (int64_t)g.hidden >= (int64_t)1 << 31)
+        return fail(MLP_ERR_UNSUPPORTED, "the per-equation baselines index batch x hidden with int32 "
+                    "(batch %d x hidden %d is too large)", batch, g.hidden);
+    if (per_equation && variant != MLP_VARIANT_UNFUSED && rows > 65535LL * 16)
+        return fail(MLP_ERR_UNSUPPORTED, "the paper's 16x16-block kernels put the batch rows in gridDim.y (batch <= 1,048,560)");
+    return MLP_OK;
+}
+
+// every entry of a host batch-order table must name a batch of the epoch
+int check_order_host(const int32_t* order, int64_t count, int64_t nb) {
+    for (int64_t k = 0; k < count; ++k)
+        if (order[k] < 0 || order[k] >= nb)
+            return fail(MLP_ERR_BAD_ARG, "batch_order[%lld] = %d is outside [0, %lld)", (long long)k, order[k],
+                        (long long)nb);
     return MLP_OK;
 }
 
 int train_impl(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
-               float* W1, float* W2, const int32_t* order, int variant, cudaStream_t stream) {
+               float* W1, float* W2, const int32_t* order, int variant, cudaStream_t stream,
+               unsigned long long* stats_slot = nullptr) {
     int rc = check_train_args(X, Y, n, batch, lr, epochs, W1, W2, variant);
     if (rc) return rc;
     if (epochs == 0) return MLP_OK;
     if ((rc = ensure_device())) return rc;
     if (variant == MLP_VARIANT_FUSED) {
-        const int C = effective_cluster();
+        const int C = effective_cluster(batch);
         if (!fused_supported(g.hidden, C))
             return fail(MLP_ERR_UNSUPPORTED, "cluster %d unsupported for hidden %d", C, g.hidden);
-        if (!g.stats) {
-            CK(cudaMalloc(reinterpret_cast<void**>(&g.stats), 4 * sizeof(unsigned long long)));
-            CK(cudaMemset(g.stats, 0, 4 * sizeof(unsigned long long)));
-        }
+        unsigned long long* st = stats_slot ? stats_slot : acquire_stats_slot();
+        if (!st) return cuda_fail(cudaGetLastError(), "statistics slot");
         cudaError_t e = launch_train_fused(X, Y, n, batch, lr, epochs, W1, W2, order, g.hidden, C,
-                                           g.stats, stream, &g.launches);
+                                           st, stream, &g.launches);
         if (e != cudaSuccess) return cuda_fail(e, "launch_train_fused");
         return MLP_OK;
     }
-    if (variant == MLP_VARIANT_TF32) {
-        if (!train_tf32_supported(g.hidden))
-            return fail(MLP_ERR_UNSUPPORTED, "TF32 training variant supports hidden 32..256 (got %d)", g.hidden);
-        cudaError_t e = launch_train_tf32(X, Y, n, batch, lr, epochs, W1, W2, order, g.hidden, stream, &g.launches);
-        if (e != cudaSuccess) return cuda_fail(e, "launch_train_tf32");
+    if (variant == MLP_VARIANT_TF32 || variant == MLP_VARIANT_BF16) {
+        const bool bf16 = variant == MLP_VARIANT_BF16;
+        if (!train_tc_supported(g.hidden, bf16))
+            return fail(MLP_ERR_UNSUPPORTED, "tensor-core training variant %d does not support hidden %d", variant, g.hidden);
+        unsigned long long* st = stats_slot ? stats_slot : acquire_stats_slot();
+        if (!st) return cuda_fail(cudaGetLastError(), "statistics slot");
+        cudaError_t e = launch_train_tc(X, Y, n, batch, lr, epochs, W1, W2, order, g.hidden, bf16, st, stream, &g.launches);
+        if (e != cudaSuccess) return cuda_fail(e, "launch_train_tc");
         return MLP_OK;
     }
-    // unfused baseline: the host loop needs the batch order on the host
+    // per-equation baselines: the host loop needs the batch order on the host
     if ((rc = ensure_unfused(batch > n ? (int)n : batch, g.hidden))) return rc;
     std::vector<int32_t> oh;
     if (order) {
@@ -161,8 +247,7 @@ int train_impl(const float* X, const float* Y, int64_t n, int batch, float lr, i
         oh.resize((size_t)nb * epochs);
         CK(cudaMemcpyAsync(oh.data(), order, oh.size() * 4, cudaMemcpyDeviceToHost, stream));
         CK(cudaStreamSynchronize(stream));
-        for (int32_t t : oh)
-            if (t < 0 || t >= nb) return fail(MLP_ERR_BAD_ARG, "batch_order entry %d outside [0,%lld)", t, (long long)nb);
+        if ((rc = check_order_host(oh.data(), (int64_t)oh.size(), nb))) return rc;
     }
     cudaError_t e;
     if (variant == MLP_VARIANT_UNFUSED)
@@ -176,36 +261,45 @@ int train_impl(const float* X, const float* Y, int64_t n, int batch, float lr, i
     return MLP_OK;
 }
 
-int eval_impl(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
-              double* d_out, int variant, cudaStream_t stream) {
+int check_eval_args(const float* X, const float* Y, int64_t n, const float* W1, const float* W2, int variant) {
     if (!g.init) return fail(MLP_ERR_NOT_INIT, "mlp_init has not been called");
-    if (!X || !Y || !W1 || !W2 || !d_out) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
+    if (!X || !Y || !W1 || !W2) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
     if (n < 1) return fail(MLP_ERR_BAD_ARG, "n must be >= 1 (got %lld)", (long long)n);
     if ((uintptr_t)X & 15) return fail(MLP_ERR_ALIGN, "X must be 16-byte aligned");
-    int rc = ensure_device();
-    if (rc) return rc;
-    if (variant == MLP_VARIANT_FUSED) {
-        const int grid = eval_fp32_grid(g.hidden, g.num_sms);
-        if ((rc = ensure_eval_scratch(grid))) return rc;
-        cudaError_t e = launch_eval_fp32(X, Y, n, W1, W2, g.hidden, g.eval_partials, grid, d_out,
-                                         stream, &g.launches);
-        if (e != cudaSuccess) return cuda_fail(e, "launch_eval_fp32");
-        return MLP_OK;
-    }
-    if (variant == MLP_VARIANT_TF32) {
-        if (!eval_tf32_supported(g.hidden))
-            return fail(MLP_ERR_UNSUPPORTED, "TF32 eval unsupported for hidden %d", g.hidden);
-        const int grid = g.num_sms;
-        if ((rc = ensure_eval_scratch(grid))) return rc;
-        cudaError_t e = launch_eval_tf32(X, Y, n, W1, W2, g.hidden, g.eval_partials, grid, d_out,
-                                         stream, &g.launches);
-        if (e != cudaSuccess) return cuda_fail(e, "launch_eval_tf32");
-        return MLP_OK;
-    }
-    return fail(MLP_ERR_UNSUPPORTED, "eval variant %d is not supported", variant);
+    if (variant != MLP_VARIANT_FUSED && !eval_tc_supported(g.hidden, variant))
+        return fail(MLP_ERR_UNSUPPORTED, "eval variant %d is not supported for hidden %d", variant, g.hidden);
+    return MLP_OK;
 }
 
-int ensure_host_path(int64_t n, int64_t norder) {
+// launches one eval kernel with the given workspace; the mean loss goes to *d_out
+int eval_launch(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+                double* d_out, int variant, const EvalWs& ws, cudaStream_t stream) {
+    cudaError_t e;
+    if (variant == MLP_VARIANT_FUSED)
+        e = launch_eval_fp32(X, Y, n, W1, W2, g.hidden, ws.partials, ws.ticket, eval_fp32_grid(g.hidden, g.num_sms),
+                             d_out, stream, &g.launches);
+    else
+        e = launch_eval_tc(X, Y, n, W1, W2, g.hidden, variant, ws.partials, ws.ticket, g.num_sms, d_out, stream,
+                           &g.launches);
+    if (e != cudaSuccess) return cuda_fail(e, "eval kernel launch");
+    return MLP_OK;
+}
+
+// pool-backed eval: the loss goes to *d_out (device); with d_out == nullptr it goes to the slot's own result
+// word and is copied to *h_result (host) on the same stream before the slot is released for reuse
+int eval_impl(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+              double* d_out, int variant, cudaStream_t stream, double* h_result = nullptr) {
+    int rc = check_eval_args(X, Y, n, W1, W2, variant);
+    if (rc) return rc;
+    EvalWs ws;
+    if ((rc = acquire_eval_slot(stream, &ws))) return rc;
+    if (!d_out) d_out = ws.result;
+    if ((rc = eval_launch(X, Y, n, W1, W2, d_out, variant, ws, stream))) return rc;
+    if (h_result) CK(cudaMemcpyAsync(h_result, ws.result, sizeof(double), cudaMemcpyDeviceToHost, stream));
+    return release_eval_slot(ws, stream);
+}
+
+int ensure_host_path(int64_t n, int64_t norder, int64_t nloss) {
     int rc;
     if ((rc = grow(&g.hX, &g.hX_cap, (size_t)n * kIn))) return rc;
     if ((rc = grow(&g.hY, &g.hY_cap, (size_t)n))) return rc;
@@ -218,7 +312,22 @@ int ensure_host_path(int64_t n, int64_t norder) {
     }
     g.hW2 = g.hW1 + (size_t)kIn * g.hidden;
     if (norder > 0 && (rc = grow(&g.hOrder, &g.hOrder_cap, (size_t)norder))) return rc;
+    if (nloss > 0 && (rc = grow(&g.hLoss, &g.hLoss_cap, (size_t)nloss))) return rc;
     if (!g.host_stream) CK(cudaStreamCreateWithFlags(&g.host_stream, cudaStreamNonBlocking));
+    if (!g.copy_stream) {
+        CK(cudaStreamCreateWithFlags(&g.copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < kHostChunks; ++i) CK(cudaEventCreateWithFlags(&g.chunk_ev[i], cudaEventDisableTiming));
+    }
+    return MLP_OK;
+}
+
+int check_host_train_args(const float* X_host, const float* Y_host, int64_t n, int batch, int epochs,
+                          const float* W1_host, const float* W2_host, const int32_t* order_host) {
+    if (!g.init) return fail(MLP_ERR_NOT_INIT, "mlp_init has not been called");
+    if (!X_host || !Y_host || !W1_host || !W2_host) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
+    if (n < 1 || batch < 1 || epochs < 0) return fail(MLP_ERR_BAD_ARG, "bad n/batch/epochs");
+    const int64_t nb = (n + batch - 1) / batch;
+    if (order_host) return check_order_host(order_host, nb * epochs, nb);      // before anything is copied
     return MLP_OK;
 }
 
@@ -260,15 +369,12 @@ int mlp_train_ex(const float* X, const float* Y, int64_t n, int batch, float lr,
 
 double mlp_eval_loss(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
                      void* stream) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    int rc = ensure_device();
-    if (!rc) rc = ensure_eval_scratch(g.num_sms);
-    if (rc) return NAN;
-    rc = eval_impl(X, Y, n, W1, W2, g.eval_out, MLP_VARIANT_FUSED, (cudaStream_t)stream);
-    if (rc) return NAN;
     double h = NAN;
-    cudaError_t e = cudaMemcpyAsync(&h, g.eval_out, sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (eval_impl(X, Y, n, W1, W2, nullptr, MLP_VARIANT_FUSED, (cudaStream_t)stream, &h)) return NAN;
+    }
+    const cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
     if (e != cudaSuccess) { cuda_fail(e, "mlp_eval_loss readback"); return NAN; }
     return h;
 }
@@ -276,7 +382,33 @@ double mlp_eval_loss(const float* X, const float* Y, int64_t n, const float* W1,
 int mlp_eval_loss_async(const float* X, const float* Y, int64_t n, const float* W1,
                         const float* W2, double* d_out, int variant, void* stream) {
     std::lock_guard<std::mutex> lk(g_mu);
+    if (!d_out) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
     return eval_impl(X, Y, n, W1, W2, d_out, variant, (cudaStream_t)stream);
+}
+
+size_t mlp_eval_workspace_bytes(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (ensure_device()) return 0;
+    return sizeof(double) * eval_ws_doubles();
+}
+
+int mlp_eval_loss_ws(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+                     double* d_out, int variant, void* workspace, size_t workspace_bytes, void* stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!d_out || !workspace) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
+    int rc = check_eval_args(X, Y, n, W1, W2, variant);
+    if (rc) return rc;
+    if ((rc = ensure_device())) return rc;
+    if ((uintptr_t)workspace & 7) return fail(MLP_ERR_ALIGN, "workspace must be 8-byte aligned");
+    if (workspace_bytes < sizeof(double) * eval_ws_doubles())
+        return fail(MLP_ERR_BAD_ARG, "workspace too small: %zu < %zu bytes", workspace_bytes,
+                    sizeof(double) * eval_ws_doubles());
+    EvalWs ws;
+    ws.partials = static_cast<double*>(workspace);
+    ws.ticket = reinterpret_cast<unsigned int*>(ws.partials + g.num_sms);
+    ws.result = ws.partials + g.num_sms + 1;
+    ws.slot = -1;
+    return eval_launch(X, Y, n, W1, W2, d_out, variant, ws, (cudaStream_t)stream);
 }
 
 int mlp_train_rows(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
@@ -286,13 +418,18 @@ int mlp_train_rows(const float* X, const float* Y, int64_t n, int batch, float l
     int rc = check_train_args(X, Y, n, batch, lr, epochs, W1, W2, MLP_VARIANT_FUSED);
     if (rc) return rc;
     if (n > 0x7fffffffLL / 8) return fail(MLP_ERR_BAD_ARG, "n too large for int32 row indices");
+    if (epochs == 0) return MLP_OK;
     if ((rc = grow(&g.shufX, &g.shufX_cap, (size_t)n * kIn))) return rc;
     if ((rc = grow(&g.shufY, &g.shufY_cap, (size_t)n))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* slot = acquire_stats_slot();
+    if (!slot) return cuda_fail(cudaGetLastError(), "statistics slot");
+    CK(cudaMemsetAsync(slot + 5, 0, sizeof(unsigned long long), st));     // bad row_order entries of this call
     for (int e = 0; e < epochs; ++e) {
-        cudaError_t err = launch_gather_rows(X, Y, row_order + (int64_t)e * n, g.shufX, g.shufY, n, st, &g.launches);
+        cudaError_t err = launch_gather_rows(X, Y, row_order + (int64_t)e * n, g.shufX, g.shufY, n, slot + 5, st,
+                                             &g.launches);
         if (err != cudaSuccess) return cuda_fail(err, "launch_gather_rows");
-        if ((rc = train_impl(g.shufX, g.shufY, n, batch, lr, 1, W1, W2, nullptr, MLP_VARIANT_FUSED, st))) return rc;
+        if ((rc = train_impl(g.shufX, g.shufY, n, batch, lr, 1, W1, W2, nullptr, MLP_VARIANT_FUSED, st, slot))) return rc;
     }
     return MLP_OK;
 }
@@ -300,14 +437,19 @@ int mlp_train_rows(const float* X, const float* Y, int64_t n, int batch, float l
 int mlp_train_host(const float* X_host, const float* Y_host, int64_t n, int batch, float lr,
                    int epochs, float* W1_host, float* W2_host, const int32_t* order_host,
                    int variant) {
+    return mlp_fit_host(X_host, Y_host, n, batch, lr, epochs, W1_host, W2_host, order_host, variant,
+                        MLP_VARIANT_FUSED, nullptr);
+}
+
+int mlp_fit_host(const float* X_host, const float* Y_host, int64_t n, int batch, float lr, int epochs,
+                 float* W1_host, float* W2_host, const int32_t* order_host, int variant,
+                 int eval_variant, double* epoch_loss_host) {
     std::lock_guard<std::mutex> lk(g_mu);
-    if (!g.init) return fail(MLP_ERR_NOT_INIT, "mlp_init has not been called");
-    if (!X_host || !Y_host || !W1_host || !W2_host) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
-    if (n < 1 || batch < 1 || epochs < 0) return fail(MLP_ERR_BAD_ARG, "bad n/batch/epochs");
+    int rc = check_host_train_args(X_host, Y_host, n, batch, epochs, W1_host, W2_host, order_host);
+    if (rc) return rc;
     const int64_t nb = (n + batch - 1) / batch;
     const int64_t norder = order_host ? nb * epochs : 0;
-    int rc = ensure_host_path(n, norder);
-    if (rc) return rc;
+    if ((rc = ensure_host_path(n, norder, epoch_loss_host ? epochs : 0))) return rc;
     cudaStream_t st = g.host_stream;
     const size_t n1 = (size_t)kIn * g.hidden;
     CK(cudaMemcpyAsync(g.hX, X_host, (size_t)n * kIn * 4, cudaMemcpyHostToDevice, st));
@@ -315,8 +457,22 @@ int mlp_train_host(const float* X_host, const float* Y_host, int64_t n, int batc
     CK(cudaMemcpyAsync(g.hW1, W1_host, n1 * 4, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(g.hW2, W2_host, (size_t)g.hidden * 4, cudaMemcpyHostToDevice, st));
     if (norder) CK(cudaMemcpyAsync(g.hOrder, order_host, (size_t)norder * 4, cudaMemcpyHostToDevice, st));
-    rc = train_impl(g.hX, g.hY, n, batch, lr, epochs, g.hW1, g.hW2, norder ? g.hOrder : nullptr, variant, st);
-    if (rc) return rc;
+    if (!epoch_loss_host) {
+        // the whole job in one launch (no per-epoch evaluation requested)
+        if ((rc = train_impl(g.hX, g.hY, n, batch, lr, epochs, g.hW1, g.hW2, norder ? g.hOrder : nullptr, variant, st)))
+            return rc;
+    } else {
+        // BASELINE.json configs[2]: "a full-dataset eval-loss pass after each epoch": one training launch
+        // and one eval launch per epoch, all asynchronous; the losses come back with the weights
+        for (int e = 0; e < epochs; ++e) {
+            if ((rc = train_impl(g.hX, g.hY, n, batch, lr, 1, g.hW1, g.hW2, norder ? g.hOrder + (int64_t)e * nb : nullptr,
+                                 variant, st)))
+                return rc;
+            if ((rc = eval_impl(g.hX, g.hY, n, g.hW1, g.hW2, g.hLoss + e, eval_variant, st))) return rc;
+        }
+        if (epochs > 0)
+            CK(cudaMemcpyAsync(epoch_loss_host, g.hLoss, sizeof(double) * epochs, cudaMemcpyDeviceToHost, st));
+    }
     CK(cudaMemcpyAsync(W1_host, g.hW1, n1 * 4, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(W2_host, g.hW2, (size_t)g.hidden * 4, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -328,20 +484,40 @@ double mlp_eval_loss_host(const float* X_host, const float* Y_host, int64_t n,
     std::lock_guard<std::mutex> lk(g_mu);
     if (!g.init) { fail(MLP_ERR_NOT_INIT, "mlp_init has not been called"); return NAN; }
     if (!X_host || !Y_host || !W1_host || !W2_host || n < 1) { fail(MLP_ERR_BAD_ARG, "bad argument"); return NAN; }
-    if (ensure_host_path(n, 0) || ensure_device() || ensure_eval_scratch(g.num_sms)) return NAN;
-    cudaStream_t st = g.host_stream;
+    // Pipelined: X/Y go to the device in chunks on a copy stream; the eval kernel of chunk k starts on
+    // the compute stream as soon as chunk k has landed, while chunk k+1 is still in flight.  Each
+    // chunk's kernel returns the mean over its rows (eq. 4 restricted to the chunk); the dataset loss
+    // is the row-weighted mean of those, formed here in chunk order (deterministic).
+    int64_t chunk = kChunkRows;
+    while ((n + chunk - 1) / chunk > kHostChunks) chunk *= 2;
+    const int nchunks = (int)((n + chunk - 1) / chunk);
+    if (ensure_host_path(n, 0, nchunks) || ensure_device()) return NAN;
+    cudaStream_t st = g.host_stream, cs = g.copy_stream;
     const size_t n1 = (size_t)kIn * g.hidden;
-    cudaError_t e = cudaMemcpyAsync(g.hX, X_host, (size_t)n * kIn * 4, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(g.hY, Y_host, (size_t)n * 4, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(g.hW1, W1_host, n1 * 4, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(g.hW1, W1_host, n1 * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(g.hW2, W2_host, (size_t)g.hidden * 4, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) { cuda_fail(e, "mlp_eval_loss_host H2D"); return NAN; }
-    if (eval_impl(g.hX, g.hY, n, g.hW1, g.hW2, g.eval_out, variant, st)) return NAN;
-    double h = NAN;
-    e = cudaMemcpyAsync(&h, g.eval_out, sizeof(double), cudaMemcpyDeviceToHost, st);
+    for (int k = 0; k < nchunks; ++k) {
+        const int64_t r0 = (int64_t)k * chunk, rows = (n - r0 < chunk) ? n - r0 : chunk;
+        e = cudaMemcpyAsync(g.hX + r0 * kIn, X_host + r0 * kIn, (size_t)rows * kIn * 4, cudaMemcpyHostToDevice, cs);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(g.hY + r0, Y_host + r0, (size_t)rows * 4, cudaMemcpyHostToDevice, cs);
+        if (e == cudaSuccess) e = cudaEventRecord(g.chunk_ev[k], cs);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, g.chunk_ev[k], 0);
+        if (e != cudaSuccess) { cuda_fail(e, "mlp_eval_loss_host H2D"); return NAN; }
+        if (eval_impl(g.hX + r0 * kIn, g.hY + r0, rows, g.hW1, g.hW2, g.hLoss + k, variant, st)) return NAN;
+    }
+    std::vector<double> h((size_t)nchunks);
+    e = cudaMemcpyAsync(h.data(), g.hLoss, sizeof(double) * nchunks, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
     if (e != cudaSuccess) { cuda_fail(e, "mlp_eval_loss_host D2H"); return NAN; }
-    return h;
+    if (nchunks == 1) return h[0];
+    double sse = 0.0;
+    for (int k = 0; k < nchunks; ++k) {
+        const int64_t r0 = (int64_t)k * chunk, rows = (n - r0 < chunk) ? n - r0 : chunk;
+        sse += h[k] * (double)rows;
+    }
+    return sse / (double)n;
 }
 
 int mlp_set_cluster(int cluster) {
@@ -356,17 +532,33 @@ int mlp_set_cluster(int cluster) {
 
 int mlp_get_cluster(void) {
     std::lock_guard<std::mutex> lk(g_mu);
-    return g.init ? effective_cluster() : 0;
+    return g.init ? effective_cluster(256) : 0;
+}
+
+int mlp_get_cluster_for(int batch) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return g.init && batch >= 1 ? effective_cluster(batch) : 0;
 }
 
 int mlp_get_train_stats(double out[4]) {
     std::lock_guard<std::mutex> lk(g_mu);
     if (!out) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
-    if (!g.stats) return fail(MLP_ERR_NOT_INIT, "no fused training call has run yet");
+    if (!g.stats || g.stats_latest < 0) return fail(MLP_ERR_NOT_INIT, "no fused training call has run yet");
     unsigned long long h[4];
-    CK(cudaMemcpy(h, g.stats, sizeof(h), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(h, g.stats + (size_t)g.stats_latest * kStatWords, sizeof(h), cudaMemcpyDeviceToHost));
     for (int i = 0; i < 4; ++i) out[i] = (double)h[i];
     return MLP_OK;
+}
+
+int64_t mlp_train_order_errors(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g.stats || g.stats_latest < 0) return 0;
+    unsigned long long h[2];
+    if (cudaMemcpy(h, g.stats + (size_t)g.stats_latest * kStatWords + 4, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cuda_fail(cudaGetLastError(), "mlp_train_order_errors");
+        return -1;
+    }
+    return (int64_t)(h[0] + h[1]);
 }
 
 int64_t mlp_launch_count(void) {
@@ -376,13 +568,19 @@ int64_t mlp_launch_count(void) {
 
 const char* mlp_last_error(void) { return g_err; }
 
-const char* mlp_version(void) { return "libmlp_b200 0.1 (sm_100a)"; }
+const char* mlp_version(void) { return "libmlp_b200 0.2 (sm_100a)"; }
 
 void mlp_shutdown(void) {
     std::lock_guard<std::mutex> lk(g_mu);
-    void* ptrs[] = {g.eval_partials, g.eval_out, g.stats, g.unf.Z1, g.unf.Hact, g.unf.dZ1,
-                    g.unf.Ypred, g.unf.dZ2, g.unf.dW1, g.unf.dW2, g.priorXT, g.priorHT, g.shufX, g.shufY, g.hX, g.hY, g.hW1, g.hOrder};
+    void* ptrs[] = {g.eval_pool, g.stats, g.unf.Z1, g.unf.Hact, g.unf.dZ1,
+                    g.unf.Ypred, g.unf.dZ2, g.unf.dW1, g.unf.dW2, g.priorXT, g.priorHT, g.shufX, g.shufY, g.hX, g.hY,
+                    g.hW1, g.hOrder, g.hLoss};
     for (void* p : ptrs) if (p) cudaFree(p);
+    if (g.eval_pool) for (int i = 0; i < kEvalSlots; ++i) if (g.eval_done[i]) cudaEventDestroy(g.eval_done[i]);
+    if (g.copy_stream) {
+        for (int i = 0; i < kHostChunks; ++i) if (g.chunk_ev[i]) cudaEventDestroy(g.chunk_ev[i]);
+        cudaStreamDestroy(g.copy_stream);
+    }
     if (g.host_stream) cudaStreamDestroy(g.host_stream);
     const bool init = g.init; const uint64_t seed = g.seed;
     const int in = g.in, hidden = g.hidden, out = g.out, cluster = g.cluster;

@@ -7,8 +7,6 @@
 
 namespace mlp {
 
-
-
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
@@ -118,5 +116,27 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
+
+// Sum NV per-lane values across the L lanes of a sample group.  On return v[0] of the lane with
+// (lu & (NV-1)) == k holds the total of original entry k (transposing butterfly: each step halves
+// the number of live values, so the whole reduction costs NV-1 + log2(L/NV) shuffles).
+template <int NV, int L, int O = 1>
+struct GroupReduce {
+    static __device__ __forceinline__ void run(float* v, int lu) {
+        if constexpr (NV > 1) {
+            const bool up = (lu & O) != 0;
+#pragma unroll
+            for (int k = 0; k < NV / 2; ++k) {
+                const float keep = up ? v[2 * k + 1] : v[2 * k];
+                const float send = up ? v[2 * k] : v[2 * k + 1];
+                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, O);
+            }
+            GroupReduce<NV / 2, L, O * 2>::run(v, lu);
+        } else if constexpr (O < L) {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], O);
+            GroupReduce<1, L, O * 2>::run(v, lu);
+        }
+    }
+};
 
 }  // namespace mlp

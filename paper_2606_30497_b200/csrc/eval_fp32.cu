@@ -20,25 +20,6 @@ namespace {
 constexpr int kTileRows = 128;
 constexpr int kStages = 4;
 
-template <int NV, int L, int O = 1>
-struct LaneReduce {
-    static __device__ __forceinline__ void run(float* v, int lu) {
-        if constexpr (NV > 1) {
-            const bool up = (lu & O) != 0;
-#pragma unroll
-            for (int k = 0; k < NV / 2; ++k) {
-                const float keep = up ? v[2 * k + 1] : v[2 * k];
-                const float send = up ? v[2 * k] : v[2 * k + 1];
-                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, O);
-            }
-            LaneReduce<NV / 2, L, O * 2>::run(v, lu);
-        } else if constexpr (O < L) {
-            v[0] += __shfl_xor_sync(0xffffffffu, v[0], O);
-            LaneReduce<1, L, O * 2>::run(v, lu);
-        }
-    }
-};
-
 template <int H>
 struct EvalCfg {
     static constexpr int LPS = H / 4;                               // lanes per row (four hidden units per lane)
@@ -154,7 +135,7 @@ k_eval_fp32(const float* __restrict__ X, const float* __restrict__ Y, long long 
                 for (int j = 0; j < 4; ++j) h[j] = fmaxf(hsum2(a[j]), 0.f);             // eq. 2
                 pv[k] = fmaf(h[1], w2r[1], h[0] * w2r[0]) + fmaf(h[3], w2r[3], h[2] * w2r[2]);   // eq. 3
             }
-            LaneReduce<CH, LW>::run(pv, lu);
+            GroupReduce<CH, LW>::run(pv, lu);
             float yp = pv[0];
             if constexpr (WPG > 1) {
                 float* rbuf = red + ((chunk_par * G + g) * WPG) * CH;
@@ -205,12 +186,11 @@ k_eval_fp32(const float* __restrict__ X, const float* __restrict__ Y, long long 
 
 template <int H>
 cudaError_t launch_h(const float* X, const float* Y, long long n, const float* W1, const float* W2,
-                     double* partials, int grid, double* d_out, cudaStream_t stream) {
+                     double* partials, unsigned int* ticket, int grid, double* d_out, cudaStream_t stream) {
     auto kern = k_eval_fp32<H>;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)EvalCfg<H>::smem);
     if (err != cudaSuccess) return err;
-    unsigned int* ticket = reinterpret_cast<unsigned int*>(partials + grid);
     kern<<<grid, EvalCfg<H>::NT, EvalCfg<H>::smem, stream>>>(X, Y, n, W1, W2, partials, ticket, d_out);
     return cudaGetLastError();
 }
@@ -223,16 +203,16 @@ int eval_fp32_grid(int hidden, int num_sms) {
 }
 
 cudaError_t launch_eval_fp32(const float* X, const float* Y, int64_t n, const float* W1,
-                             const float* W2, int hidden, double* partials, int grid,
+                             const float* W2, int hidden, double* partials, unsigned int* ticket, int grid,
                              double* d_out, cudaStream_t stream, int64_t* launches) {
     cudaError_t err;
     switch (hidden) {
-        case 32: err = launch_h<32>(X, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 64: err = launch_h<64>(X, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 128: err = launch_h<128>(X, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 256: err = launch_h<256>(X, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 512: err = launch_h<512>(X, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 1024: err = launch_h<1024>(X, Y, n, W1, W2, partials, grid, d_out, stream); break;
+        case 32: err = launch_h<32>(X, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 64: err = launch_h<64>(X, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 128: err = launch_h<128>(X, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 256: err = launch_h<256>(X, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 512: err = launch_h<512>(X, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 1024: err = launch_h<1024>(X, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
         default: return cudaErrorInvalidValue;
     }
     if (err == cudaSuccess) ++*launches;

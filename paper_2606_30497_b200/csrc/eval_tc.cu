@@ -23,8 +23,7 @@
 // hidden > 256: 256-column slices of the same X tile alternate between the two accumulators.
 #include <cuda.h>
 
-#include "common.cuh"
-#include "internal.h"
+#include "tc_common.cuh"
 
 namespace mlp {
 namespace {
@@ -33,50 +32,6 @@ constexpr int kTile = 128;           // rows per MMA (M)
 constexpr int kStages = 6;           // X ring depth (6 x 16 KB)
 constexpr int kEvalThreads = 352;    // producer + MMA (even tiles) + 8 epilogue warps + MMA (odd tiles)
 constexpr uint32_t kTileBytes = kTile * kIn * 4;
-
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1,
-                                            uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-        ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
-                 : "memory");
-}
-// D[tmem] (+)= A[smem desc] * B[smem desc], fp32 operands read as TF32
-__device__ __forceinline__ void mma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                         uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-// 32 lanes x 32 consecutive columns: thread t of the warp gets lane (base + t), columns c..c+31
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
-          "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
-          "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
-          "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr)
-        : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-
-// K-major, 128-byte-swizzled operand descriptor (8-row x 128-byte atoms, 1024 bytes apart)
-__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
-    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
-}
 
 // Hidden widths above 256 (one MMA N-extent, half of TMEM) are processed as NS = H/256 column
 // slices per tile: the X tile is read from HBM once, slice sl of a tile goes to accumulator
@@ -366,13 +321,12 @@ EncodeTiledFn encode_tiled() {
 
 template <int H>
 cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const float* W1, const float* W2,
-                     double* partials, int grid, double* d_out, cudaStream_t stream) {
+                     double* partials, unsigned int* ticket, int grid, double* d_out, cudaStream_t stream) {
     auto kern = k_eval_tf32<H>;
     const size_t smem = (size_t)H * kIn * 4 + (size_t)eval_stages(H) * kTileBytes + (size_t)H * 4 + 2 * kTile * 4 + 32 * 4 +
                         8 * (2 * kStages + 16) + 8 * 8 + 4 * H + 32 + 4 + 16;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
-    unsigned int* ticket = reinterpret_cast<unsigned int*>(partials + grid);
     kern<<<grid, kEvalThreads, smem, stream>>>(tmap, Y, n, W1, W2, partials, ticket, d_out);
     return cudaGetLastError();
 }
@@ -391,13 +345,15 @@ bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows) {
                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-bool eval_tf32_supported(int hidden) {
+bool eval_tc_supported(int hidden, int variant) {
+    if (variant != 2 /* MLP_VARIANT_TF32 */) return false;
     return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256 || hidden == 512 || hidden == 1024;
 }
 
-cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
-                             int hidden, double* partials, int grid, double* d_out, cudaStream_t stream,
-                             int64_t* launches) {
+cudaError_t launch_eval_tc(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+                           int hidden, int variant, double* partials, unsigned int* ticket, int grid, double* d_out,
+                           cudaStream_t stream, int64_t* launches) {
+    if (!eval_tc_supported(hidden, variant)) return cudaErrorInvalidValue;
     if (n > 0x7fffffffLL - kTile) return cudaErrorInvalidValue;      // TMA coordinates are int32
     // X as a 2-D tensor [n rows][32 floats]; box = one 128-row tile; 128-byte swizzle = the layout
     // tcgen05.mma reads a K-major operand in (a row is exactly one 128-byte swizzle span).
@@ -405,12 +361,12 @@ cudaError_t launch_eval_tf32(const float* X, const float* Y, int64_t n, const fl
     if (!make_x_tensormap(&tmap, X, n, kTile)) return cudaErrorNotSupported;
     cudaError_t err;
     switch (hidden) {
-        case 32: err = launch_h<32>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 64: err = launch_h<64>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 128: err = launch_h<128>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 256: err = launch_h<256>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 512: err = launch_h<512>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
-        case 1024: err = launch_h<1024>(tmap, Y, n, W1, W2, partials, grid, d_out, stream); break;
+        case 32: err = launch_h<32>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 64: err = launch_h<64>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 128: err = launch_h<128>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 256: err = launch_h<256>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 512: err = launch_h<512>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 1024: err = launch_h<1024>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
         default: return cudaErrorInvalidValue;
     }
     if (err == cudaSuccess) ++*launches;

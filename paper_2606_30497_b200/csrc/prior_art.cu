@@ -96,6 +96,7 @@ cudaError_t launch_train_prior(bool tiled, const float* X, const float* Y, int64
             const int mh = m * H;
             if (!tiled) {
                 k_mm_naive<false><<<grid2(m, H), tb, 0, stream>>>(Xb, W1, s.Z1, m, kIn, H);           // eq. 1
+                { const cudaError_t e1 = cudaGetLastError(); if (e1 != cudaSuccess) return e1; }
                 k_relu_p<<<(mh + 255) / 256, 256, 0, stream>>>(s.Z1, s.Hact, mh);                     // eq. 2
                 k_mm_naive<false><<<grid2(m, 1), tb, 0, stream>>>(s.Hact, W2, s.Ypred, m, H, 1);      // eq. 3
                 k_dz2_p<<<(m + 255) / 256, 256, 0, stream>>>(s.Ypred, Yb, s.dZ2, m);                  // eq. 5
@@ -106,6 +107,7 @@ cudaError_t launch_train_prior(bool tiled, const float* X, const float* Y, int64
                 *launches += 8;
             } else {
                 k_mm_tiled<true><<<grid2(m, H), tb, 0, stream>>>(Xb, W1, s.Hact, m, kIn, H);          // eqs. 1-2
+                { const cudaError_t e1 = cudaGetLastError(); if (e1 != cudaSuccess) return e1; }
                 k_mm_tiled<false><<<grid2(m, 1), tb, 0, stream>>>(s.Hact, W2, s.Ypred, m, H, 1);      // eq. 3
                 k_dz2_p<<<(m + 255) / 256, 256, 0, stream>>>(s.Ypred, Yb, s.dZ2, m);                  // eq. 5
                 k_transpose<<<grid2(m, H), tb, 0, stream>>>(s.Hact, HT, m, H);

@@ -58,28 +58,6 @@ struct TrainParams {
     float scale_last;   // 2 / m_last
 };
 
-// Sum NV per-lane values across the L lanes of a sample group.  On return v[0] of the lane with
-// (lu & (NV-1)) == k holds the total of original entry k (transposing butterfly: each step halves
-// the number of live values, so the whole reduction costs NV-1 + log2(L/NV) shuffles).
-template <int NV, int L, int O = 1>
-struct GroupReduce {
-    static __device__ __forceinline__ void run(float* v, int lu) {
-        if constexpr (NV > 1) {
-            const bool up = (lu & O) != 0;
-#pragma unroll
-            for (int k = 0; k < NV / 2; ++k) {
-                const float keep = up ? v[2 * k + 1] : v[2 * k];
-                const float send = up ? v[2 * k] : v[2 * k + 1];
-                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, O);
-            }
-            GroupReduce<NV / 2, L, O * 2>::run(v, lu);
-        } else if constexpr (O < L) {
-            v[0] += __shfl_xor_sync(0xffffffffu, v[0], O);
-            GroupReduce<1, L, O * 2>::run(v, lu);
-        }
-    }
-};
-
 template <int S, int BT, int NSPLIT, int C>
 __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p) {
     constexpr int LPS = S / 4;            // lanes per sample row
@@ -135,7 +113,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     const long long total = p.total_steps;
     // batch of a step: the order table, else sequential; `seq` counts steps modulo nb without division
     int seq = 0;                                      // (step + 2) % nb for the look-ahead below
-    auto batch_index = [&](long long step, int sq) -> int { return p.order ? __ldg(p.order + step) : sq; };
+    unsigned long long bad_order = 0;     // batch_order entries outside [0, nb): clamped, counted, reported
+    auto batch_index = [&](long long step, int sq) -> int {
+        if (!p.order) return sq;
+        const int t = __ldg(p.order + step);
+        if ((unsigned)t < (unsigned)p.nbi) return t;
+        ++bad_order;
+        return t < 0 ? 0 : p.nbi - 1;
+    };
     auto rows_of = [&](int t) -> int { return t == p.nbi - 1 ? p.m_last : p.B; };
     // producer (one thread): bring `rows` rows starting at global row g0 into ring stage nbuf
     auto issue_tile = [&](long long g0, int rows, unsigned nbuf) {
@@ -450,6 +435,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
         p.stats[1] = globaltimer_ns() - ns0;
         p.stats[2] = (unsigned long long)total;
         p.stats[3] = C;
+        p.stats[4] = bad_order;
     }
     cluster_sync_all();        // no CTA exits while peers may still push into its shared memory
 }
@@ -530,7 +516,8 @@ bool fused_supported(int hidden, int cluster) {
     return S == 32 || S == 64;
 }
 
-int fused_default_cluster(int hidden) {
+int fused_default_cluster(int hidden, int batch) {
+    (void)batch;
     switch (hidden) {
         case 32: return 1;
         case 64: return 2;

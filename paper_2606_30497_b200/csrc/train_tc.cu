@@ -24,8 +24,7 @@
 // All operands are K-major with the 128-byte swizzle (the conventions of eval_tf32.cu).
 #include <cuda.h>
 
-#include "common.cuh"
-#include "internal.h"
+#include "tc_common.cuh"
 
 namespace mlp {
 namespace {
@@ -50,47 +49,8 @@ struct TcParams {
     float* W2;
     const int* order;
     int H;
+    unsigned long long* stats;   // [4] = batch_order entries outside [0, nb) (clamped and counted)
 };
-
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-        ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
-        : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                         uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
-          "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
-          "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
-          "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr)
-        : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// K-major, 128-byte-swizzled operand descriptor (8-row x 128-byte atoms, 1024 bytes apart)
-__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
-    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
-}
-// byte offset of the 16-byte chunk c of row r in a [rows][128 B] tile with the 128-byte swizzle
-__device__ __forceinline__ int swz(int r, int c) { return r * 128 + ((c ^ (r & 7)) << 4); }
 
 template <int C>
 __global__ void __launch_bounds__(kThreads, 1)
@@ -154,7 +114,14 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
     const long long total = p.total_steps;
     int seq = 0;
-    auto batch_index = [&](long long step, int sq) -> int { return p.order ? __ldg(p.order + step) : sq; };
+    unsigned long long bad_order = 0;     // batch_order entries outside [0, nb): clamped, counted, reported
+    auto batch_index = [&](long long step, int sq) -> int {
+        if (!p.order) return sq;
+        const int t = __ldg(p.order + step);
+        if ((unsigned)t < (unsigned)p.nbi) return t;
+        ++bad_order;
+        return t < 0 ? 0 : p.nbi - 1;
+    };
     auto rows_of = [&](int t) -> int { return t == p.nbi - 1 ? p.m_last : p.B; };
     auto issue_tile = [&](long long g0, unsigned nbuf) {      // one thread; the box is always 256 rows
         mbar_arrive_expect_tx(bar_full + 8 * nbuf, kXBytes);  // rows past n are zero-filled, still counted
@@ -351,6 +318,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
         for (int i = 0; i < kIn; ++i) p.W1[(size_t)i * H + crank * S + wu] = wrow[i];
     }
     if (tid < S) p.W2[crank * S + tid] = W2s[tid];
+    if (crank == 0 && tid == 0 && p.stats) { p.stats[2] = (unsigned long long)total; p.stats[3] = C; p.stats[4] = bad_order; }
     tc_fence_before();
     __syncthreads();
     if (warp == 0) {
@@ -362,14 +330,15 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
 }  // namespace
 
-bool train_tf32_supported(int hidden) {
+bool train_tc_supported(int hidden, bool bf16) {
+    if (bf16) return false;
     return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256;
 }
 
-cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
-                              float* W1, float* W2, const int32_t* order, int hidden,
-                              cudaStream_t stream, int64_t* launches) {
-    if (!train_tf32_supported(hidden) || n > 0x7fffffffLL - kBT) return cudaErrorInvalidValue;
+cudaError_t launch_train_tc(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
+                            float* W1, float* W2, const int32_t* order, int hidden, bool bf16,
+                            unsigned long long* stats, cudaStream_t stream, int64_t* launches) {
+    if (!train_tc_supported(hidden, bf16) || n > 0x7fffffffLL - kBT) return cudaErrorInvalidValue;
     const int C = hidden / kS;
     TcParams p;
     p.Y = Y; p.n = n; p.B = batch; p.lr = lr;
@@ -379,7 +348,7 @@ cudaError_t launch_train_tf32(const float* X, const float* Y, int64_t n, int bat
     p.m_last = (int)(n - (nb - 1) * batch);
     p.scale_full = 2.0f / (float)batch;
     p.scale_last = 2.0f / (float)p.m_last;
-    p.W1 = W1; p.W2 = W2; p.order = order; p.H = hidden;
+    p.W1 = W1; p.W2 = W2; p.order = order; p.H = hidden; p.stats = stats;
     if (p.total_steps == 0) return cudaSuccess;
     alignas(64) CUtensorMap tmap;
     if (!make_x_tensormap(&tmap, X, n, kBT)) return cudaErrorNotSupported;

@@ -11,8 +11,8 @@ namespace {
 // eq. 1: Z1[b][j] = sum_i X[b][i] W1[i][j]          one thread per output element
 __global__ void k_fwd1(const float* __restrict__ X, const float* __restrict__ W1,
                        float* __restrict__ Z1, int m, int H) {
-    int j = blockIdx.x * blockDim.x + threadIdx.x;
-    int b = blockIdx.y;
+    int j = blockIdx.y * blockDim.x + threadIdx.x;   // rows in gridDim.x (no 65,535 limit)
+    int b = blockIdx.x;
     if (j >= H || b >= m) return;
     float s = 0.f;
     for (int i = 0; i < kIn; ++i) s = fmaf(X[(size_t)b * kIn + i], W1[(size_t)i * H + j], s);
@@ -96,12 +96,16 @@ __global__ void k_init_weights(unsigned long long seed, int H, float* __restrict
 // float4 per thread, eight threads per 128-byte row
 __global__ void k_gather_rows(const float* __restrict__ X, const float* __restrict__ Y,
                               const int* __restrict__ perm, float* __restrict__ Xp,
-                              float* __restrict__ Yp, long long n) {
+                              float* __restrict__ Yp, long long n, unsigned long long* __restrict__ bad) {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long r = e >> 3;
     if (r >= n) return;
     const int c = (int)(e & 7);
-    const long long src = perm[r];
+    long long src = perm[r];
+    if (src < 0 || src >= n) {                      // row_order entry outside [0, n): clamped, counted, reported
+        if (c == 0) atomicAdd(bad, 1ull);
+        src = src < 0 ? 0 : n - 1;
+    }
     reinterpret_cast<float4*>(Xp)[e] = __ldg(reinterpret_cast<const float4*>(X) + src * 8 + c);
     if (c == 0) Yp[r] = __ldg(Y + src);
 }
@@ -109,9 +113,9 @@ __global__ void k_gather_rows(const float* __restrict__ X, const float* __restri
 }  // namespace
 
 cudaError_t launch_gather_rows(const float* X, const float* Y, const int32_t* perm, float* Xp, float* Yp,
-                               int64_t n, cudaStream_t stream, int64_t* launches) {
+                               int64_t n, unsigned long long* bad, cudaStream_t stream, int64_t* launches) {
     const long long total = (long long)n * 8;
-    k_gather_rows<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(X, Y, perm, Xp, Yp, n);
+    k_gather_rows<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(X, Y, perm, Xp, Yp, n, bad);
     ++*launches;
     return cudaGetLastError();
 }
@@ -138,7 +142,11 @@ cudaError_t launch_train_unfused(const float* X, const float* Y, int64_t n, int 
             const int m = (int)((n - r0) < batch ? (n - r0) : batch);
             const float* Xb = X + r0 * kIn;
             const float* Yb = Y + r0;
-            k_fwd1<<<dim3((H + tj - 1) / tj, m), tj, 0, stream>>>(Xb, W1, s.Z1, m, H);
+            k_fwd1<<<dim3(m, (H + tj - 1) / tj), tj, 0, stream>>>(Xb, W1, s.Z1, m, H);
+            {   // a failed first launch must not let the rest of the step run on stale intermediates
+                const cudaError_t e1 = cudaGetLastError();
+                if (e1 != cudaSuccess) return e1;
+            }
             k_relu<<<(m * H + 255) / 256, 256, 0, stream>>>(s.Z1, s.Hact, m * H);
             k_fwd2<<<(m + 7) / 8, 256, 0, stream>>>(s.Hact, W2, s.Ypred, m, H);
             k_dz2<<<(m + 255) / 256, 256, 0, stream>>>(s.Ypred, Yb, s.dZ2, m);
