@@ -69,6 +69,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     constexpr int XSTAGE = SPW * XBLK;    // floats per ring stage
     static_assert(LPS >= 4 && LPS <= 32 && RB % kWarps == 0 && ITER >= 1 && ITER % NSPLIT == 0, "cfg");
     static_assert(ITS >= 1 && ITS <= LPS, "transposing reduction needs ITS <= LPS");
+    // Ypred partials [2][C][BTP]: the rows of sub-group sp are shifted by sp * PADR floats, so that the
+    // SPW rows one LDS.32 of the backward pass touches (RB rows apart: the same bank when RB % 32 == 0)
+    // fall into different banks.
+    constexpr int PADR = (SPW > 1 && RB % 32 == 0) ? 32 / SPW : 0;
+    constexpr int BTP = BT + SPW * PADR;
+    static_assert(PADR == 0 || ITS <= PADR, "padding must cover the rows of one exchange sub-tile");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -78,8 +84,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 
     float* Xs = reinterpret_cast<float*>(smem_raw);          // [kRing][XSTAGE]
     constexpr int XRING = (kRing * XSTAGE + 31) / 32 * 32;    // floats; keeps what follows 128-byte aligned
-    float* ypp = Xs + XRING;                                  // [2][C][BT]
-    float* part = ypp + 2 * C * BT;                           // [kWarps][S*32]  layout [q][u][4]
+    float* ypp = Xs + XRING;                                  // [2][C][BTP]
+    float* part = ypp + 2 * C * BTP;                           // [kWarps][S*32]  layout [q][u][4]
     float* part2 = part + kWarps * S * kIn;                   // [kWarps][S]
     float* W1s = part2 + kWarps * S;                          // [S*32]          layout [q][u][4]
     float* W2s = W1s + S * kIn;                               // [S]
@@ -114,13 +120,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     // batch of a step: the order table, else sequential; `seq` counts steps modulo nb without division
     int seq = 0;                                      // (step + 2) % nb for the look-ahead below
     unsigned long long bad_order = 0;     // batch_order entries outside [0, nb): clamped, counted, reported
-    auto batch_index = [&](long long step, int sq) -> int {
+    // The table entry of step k is loaded when step k-3 starts and only looked at (range check) when
+    // step k-2 starts, so the global-load latency never sits on a step's critical path.
+    auto checked = [&](int t, int sq) -> int {
         if (!p.order) return sq;
-        const int t = __ldg(p.order + step);
         if ((unsigned)t < (unsigned)p.nbi) return t;
         ++bad_order;
         return t < 0 ? 0 : p.nbi - 1;
     };
+    auto raw_entry = [&](long long step) -> int { return (p.order && step < total) ? __ldg(p.order + step) : 0; };
     auto rows_of = [&](int t) -> int { return t == p.nbi - 1 ? p.m_last : p.B; };
     // producer (one thread): bring `rows` rows starting at global row g0 into ring stage nbuf
     auto issue_tile = [&](long long g0, int rows, unsigned nbuf) {
@@ -134,13 +142,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                          rb * 128, bar);
         }
     };
-    int t_cur = batch_index(0, 0);
-    int t_next = total > 1 ? batch_index(1, 1 % p.nbi) : 0;
+    int t_cur = checked(raw_entry(0), 0);
+    int t_next = total > 1 ? checked(raw_entry(1), 1 % p.nbi) : 0;
+    int raw2 = raw_entry(2);                          // entry of step + 2, not yet checked
     seq = 2 % p.nbi;
-    if (warp == 0 && lane == 0) {
-        const long long r0 = (long long)t_cur * p.B;
-        const int m = rows_of(t_cur);
-        issue_tile(r0, min(BT, m), 0);
+    if (warp == 0) {
+        if (elect_one()) {
+            const long long r0 = (long long)t_cur * p.B;
+            const int m = rows_of(t_cur);
+            issue_tile(r0, min(BT, m), 0);
+        }
+        __syncwarp();
     }
 
     const int rowl = warp * ITER;                     // first row of this lane inside its block
@@ -163,7 +175,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
     }
     unsigned gt = 0;   // global tile counter
     for (long long step = 0; step < total; ++step) {
-        const int t_nn = (step + 2 < total) ? batch_index(step + 2, seq) : 0;
+        const int t_nn = (step + 2 < total) ? checked(raw2, seq) : 0;
+        raw2 = raw_entry(step + 3);
         seq = seq + 1 == p.nbi ? 0 : seq + 1;
         const long long r0 = (long long)t_cur * p.B;
         const int m = rows_of(t_cur);
@@ -176,7 +189,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             const unsigned xst = gt % kRing, xph = (gt / kRing) & 1u;   // X ring stage
             const int vt = min(BT, m - j * BT);               // valid rows in this tile
             const float* Xl = Xs + xst * XSTAGE + s * XBLK + rowl * kIn;   // this lane's rows
-            const float* ypt = ypp + buf * (C * BT);
+            const float* ypt = ypp + buf * (C * BTP);
             const int row0 = s * RB + rowl;                   // tile row of this lane's first row
 
             // next tile (uniform): the rest of this batch, else the first tile of the next batch
@@ -186,20 +199,29 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                 nr0 = (long long)t_next * p.B;
                 nrows = min(BT, rows_of(t_next));
             }
-            if (warp == 0 && lane == 0) {
-                // arm this tile's exchange barriers
+            // Producer duties of warp 0: arm this tile's exchange barriers (transaction bytes that
+            // arrive before the expectation are simply counted against it) and prefetch the next X
+            // tile.  The whole warp takes the branch and one elected lane issues, so the bulk copies
+            // are plain UBLKCP instructions instead of per-lane loops.
+            auto producer_duties = [&]() {
+                if (warp == 0) {
+                    if (elect_one()) {
 #pragma unroll
-                for (int q = 0; q < NSPLIT; ++q)
-                    mbar_arrive_expect_tx(bar_yp + 8 * (buf * NSPLIT + q), C * (BT / NSPLIT) * 4);
-                if (nrows > 0) {                               // prefetch X into the other buffer
-                    // stage of tile gt+1 was last read by tile gt-2: released long ago, so
-                    // this wait never holds warp 0 back behind the other warps
-                    const unsigned g1 = gt + 1, nbuf = g1 % kRing;
-                    if (g1 >= kRing) mbar_wait(bar_empty + 8 * nbuf, ((g1 / kRing) - 1) & 1u);
-                    issue_tile(nr0, nrows, nbuf);
+                        for (int q = 0; q < NSPLIT; ++q)
+                            mbar_arrive_expect_tx(bar_yp + 8 * (buf * NSPLIT + q), C * (BT / NSPLIT) * 4);
+                        if (nrows > 0) {
+                            // the stage of tile gt+1 was last read by tile gt-2: released long ago
+                            const unsigned g1 = gt + 1, nbuf = g1 % kRing;
+                            if (g1 >= kRing) mbar_wait(bar_empty + 8 * nbuf, ((g1 / kRing) - 1) & 1u);
+                            issue_tile(nr0, nrows, nbuf);
+                        }
+                    }
+                    __syncwarp();
                 }
-            }
-            __syncwarp();
+            };
+#ifndef MLP_PRODUCER_LATE
+            producer_duties();
+#endif
             float ynext = 0.f;
             if (yholder && yrow < nrows) ynext = __ldg(p.Y + nr0 + yrow);
 
@@ -278,12 +300,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                         const float v = __shfl_sync(0xffffffffu, pv[0], (sp * LPS + k) & 31);
                         if (r < ITS * SPW) {
                             const int row = sp * RB + rowl + q * ITS + k;
-                            st_async_f32(rem_ypp + (buf * (C * BT) + crank * BT + row) * 4, v,
+                            st_async_f32(rem_ypp + (buf * (C * BTP) + crank * BTP + row + sp * PADR) * 4, v,
                                          rem_bar + 8 * (buf * NSPLIT + q));
                         }
                     }
                 }
             }
+
+#ifdef MLP_PRODUCER_LATE
+            producer_duties();
+#endif
 
             // ---------------- backward: eqs. 5-8 ----------------
             // K-split: the lane of sub-group s accumulates dW1 only for the IPS inputs
@@ -307,7 +333,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                     const float yv = __shfl_sync(0xffffffffu, ycur, s * ITER + q * ITS + kk);
                     float ypc[C];
 #pragma unroll
-                    for (int c = 0; c < C; ++c) ypc[c] = ypt[c * BT + row];
+                    for (int c = 0; c < C; ++c) ypc[c] = ypt[c * BTP + row + s * PADR];
 #pragma unroll
                     for (int o = 1; o < C; o <<= 1)                 // fixed pairwise tree over ranks
 #pragma unroll
@@ -446,7 +472,9 @@ cudaError_t launch_cfg(const TrainParams& p, cudaStream_t stream) {
     constexpr int ITER = BT / SPW / kWarps;
     constexpr int NSPLIT = ITER >= 2 ? 2 : 1;
     auto kern = k_train_fused<S, BT, NSPLIT, C>;
-    const size_t smem = sizeof(float) * ((kRing * (BT * kIn + SPW * 4) + 31) / 32 * 32 + 2 * C * BT +
+    constexpr int RB = BT / SPW;
+    constexpr int BTP = BT + ((SPW > 1 && RB % 32 == 0) ? 32 : 0);      // padded Ypred exchange rows (see the kernel)
+    const size_t smem = sizeof(float) * ((kRing * (BT * kIn + SPW * 4) + 31) / 32 * 32 + 2 * C * BTP +
                                          kWarps * S * kIn + kWarps * S + S * kIn + S) +
                         8 * (2 * kRing + 2 * NSPLIT);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
