@@ -119,8 +119,9 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 
 // Sum NV per-lane values across the L lanes of a sample group.  On return v[0] of the lane with
 // (lu & (NV-1)) == k holds the total of original entry k (transposing butterfly: each step halves
-// the number of live values, so the whole reduction costs NV-1 + log2(L/NV) shuffles).
-template <int NV, int L, int O = 1>
+// the number of live values, so the whole reduction costs NV-1 + log2(L/NV) shuffles).  The group's
+// lane index lu occupies the lane-id bits SH .. SH + log2(L) - 1.
+template <int NV, int L, int O = 1, int SH = 0>
 struct GroupReduce {
     static __device__ __forceinline__ void run(float* v, int lu) {
         if constexpr (NV > 1) {
@@ -129,12 +130,12 @@ struct GroupReduce {
             for (int k = 0; k < NV / 2; ++k) {
                 const float keep = up ? v[2 * k + 1] : v[2 * k];
                 const float send = up ? v[2 * k] : v[2 * k + 1];
-                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, O);
+                v[k] = keep + __shfl_xor_sync(0xffffffffu, send, O << SH);
             }
-            GroupReduce<NV / 2, L, O * 2>::run(v, lu);
+            GroupReduce<NV / 2, L, O * 2, SH>::run(v, lu);
         } else if constexpr (O < L) {
-            v[0] += __shfl_xor_sync(0xffffffffu, v[0], O);
-            GroupReduce<1, L, O * 2>::run(v, lu);
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], O << SH);
+            GroupReduce<1, L, O * 2, SH>::run(v, lu);
         }
     }
 };

@@ -78,7 +78,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int lu = lane % LPS, s = lane / LPS;
+    // lane <-> (row sub-group s, unit lane lu): bit 0 of s is bit 0 of the lane id, lu the next
+    // log2(LPS) bits, the other bits of s above.  With this interleaving both kinds of broadcast
+    // load cost 2 shared-memory wavefronts per LDS.128 (measured): the X loads (one address per
+    // sub-group) and the W1 register reload (one address per lu, shared by the SPW sub-groups; with
+    // lu in the low bits it costs 4).
+    constexpr int LLPS = LPS == 4 ? 2 : LPS == 8 ? 3 : LPS == 16 ? 4 : 5;
+    constexpr int LSH = SPW > 1 ? 1 : 0;                                   // position of lu in the lane id
+    const int lu = (lane >> LSH) & (LPS - 1);
+    const int s = SPW > 1 ? (lane & 1) | ((lane >> (1 + LLPS)) << 1) : 0;
+    auto lane_of = [](int sg, int l) -> int { return SPW > 1 ? (sg & 1) | (l << 1) | ((sg >> 1) << (1 + LLPS)) : l; };
     const uint32_t crank = cluster_ctarank();   // C = cluster size (template: exchange code is straight-line)
     const int H = p.H;
 
@@ -290,14 +299,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                         pv[k] = fmaf(hreg[it][1], w2r[1], hreg[it][0] * w2r[0]) +            // eq. 3
                                 fmaf(hreg[it][3], w2r[3], hreg[it][2] * w2r[2]);
                     }
-                    GroupReduce<ITS, LPS>::run(pv, lu);
+                    GroupReduce<ITS, LPS, 1, LSH>::run(pv, lu);
                     // push: lane l serves ONE destination CTA (pd) and the rows l/C, l/C + 32/C, ...
                     // of the warp's ITS*SPW totals, fetched from their holder lanes by shuffle
 #pragma unroll
                     for (int i = 0; i < NPUSH; ++i) {
                         const int r = lane / C + i * RPI;
                         const int sp = r / ITS, k = r % ITS;
-                        const float v = __shfl_sync(0xffffffffu, pv[0], (sp * LPS + k) & 31);
+                        const float v = __shfl_sync(0xffffffffu, pv[0], lane_of(sp, k) & 31);
                         if (r < ITS * SPW) {
                             const int row = sp * RB + rowl + q * ITS + k;
                             st_async_f32(rem_ypp + (buf * (C * BTP) + crank * BTP + row + sp * PADR) * 4, v,
@@ -315,7 +324,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             // K-split: the lane of sub-group s accumulates dW1 only for the IPS inputs
             // [IPS*s, IPS*(s+1)) of its four units, but over the rows of ALL sub-groups, so no
             // reduction across sub-groups is needed afterwards.  dZ1 of the other sub-groups'
-            // rows arrives by shuffle; acc[u][kk] <-> inputs IPS*s + 2kk, +1.
+            // rows arrives by shuffle; acc[u][kk] <-> inputs IPS*s + 2kk, +1.  (Rebuilding dZ1 locally
+            // from one dZ2 shuffle per row and the owner lane's 32 ReLU' bits saves 70 % of the
+            // shuffles but costs more issue slots than it frees: measured slower at C = 8.)
             constexpr int IPS = kIn / SPW;            // inputs per sub-group
             f32x2 acc[4][IPS / 2];
             const float* Xk = Xs + xst * XSTAGE + rowl * kIn + IPS * s;
@@ -344,7 +355,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 #pragma unroll
                 for (int k = 0; k < ITS; ++k) {
                     const int it = q * ITS + k;
-                    const float d = __shfl_sync(0xffffffffu, dzv, (lane & ~(LPS - 1)) | k);
+                    const float d = __shfl_sync(0xffffffffu, dzv, lane_of(s, k));
                     float e[4];
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
@@ -357,7 +368,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                         f32x2 dd[4];
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
-                            const float eo = t == 0 ? e[u] : __shfl_xor_sync(0xffffffffu, e[u], t * LPS);
+                            const float eo = t == 0 ? e[u] : __shfl_xor_sync(0xffffffffu, e[u], lane_of(t, 0));
                             dd[u] = pack2(eo, eo);
                         }
                         const ulonglong2* xrow =
@@ -406,9 +417,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 
         // ---------------- end of batch: reduce partial gradients, eq. 9 ----------------
 #pragma unroll
-        for (int o = LPS; o < 32; o <<= 1)
+        for (int sb = 1; sb < SPW; sb <<= 1)                   // across the sub-groups (bits of s)
 #pragma unroll
-            for (int u = 0; u < 4; ++u) g2[u] += __shfl_xor_sync(0xffffffffu, g2[u], o);
+            for (int u = 0; u < 4; ++u) g2[u] += __shfl_xor_sync(0xffffffffu, g2[u], lane_of(sb, 0));
         if (s == 0) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) part2[warp * S + lu + u * LPS] = g2[u];
