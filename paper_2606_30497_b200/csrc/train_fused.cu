@@ -240,64 +240,72 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
             for (int u = 0; u < 4; ++u) w2r[u] = W2s[lu + u * LPS];
             {
                 // ---------------- forward: eqs. 1-3 (W1 columns in registers) ----------------
-                // The 32 LDS.128 that bring a lane's four W1 columns back cost 4 shared-memory cycles
-                // each (no broadcast across quarter-warps), ~1,000 cycles per CTA: the first row group
-                // is therefore processed chunk-major (4 inputs at a time) with the weight chunk loaded
-                // just ahead of its FFMA2s, so the reload overlaps the FMAs instead of preceding them.
-                f32x2 w[4][16];
-                auto load_w_chunk = [&](int q) {
+                // K-split over lane pairs: of the LPS lanes of a row, lane lu and its partner lu ^ LPS/2
+                // share EIGHT hidden units (their own four each) and each takes one half of the 32
+                // inputs.  A lane thus keeps 8 columns x 16 inputs of W1 in registers (the same 128 as
+                // four whole columns), reads only half of an X row (4 LDS.128 instead of 8 for the same
+                // 64 FFMA2: every byte a load returns to the register file costs FMA issue time), and
+                // the two halves of Z1 meet by one shuffle per unit: a lane sends its partial of the
+                // partner's units and receives the partner's partial of its own (no select: register
+                // set 0 is always "my units", set 1 always "the partner's").
+                // The weight registers are reloaded every step; the first rows are processed
+                // chunk-major (4 inputs at a time) with each weight chunk loaded just ahead of its
+                // FFMA2s, so the reload overlaps the FMAs instead of preceding them.
+                constexpr int HL = LPS / 2;                  // lanes per input half
+                constexpr int RP = 1;                        // rows processed together (more only adds register pressure)
+                const int kh = lu / HL;                      // this lane's inputs: 16 kh .. 16 kh + 15
+                const int pxor = HL << LSH;                  // lane-id distance to the partner
+                f32x2 w[2][4][8];                            // [mine / partner's units][unit][input pair]
+                const float* Wh = W1s + (4 * kh * S) * 4;
+                auto load_w_chunk = [&](int c) {             // inputs 16 kh + 4c .. + 3 of the eight columns
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const ulonglong2 a =
-                            *reinterpret_cast<const ulonglong2*>(W1s + (q * S + lu + u * LPS) * 4);
-                        w[u][2 * q] = a.x; w[u][2 * q + 1] = a.y;
-                    }
-                };
-                mbar_wait(bar_full + 8 * xst, xph);
-                f32x2 z0[ITS][4];                       // Z1 accumulators of row group 0
-                load_w_chunk(0);
-#pragma unroll
-                for (int x = 0; x < 8; ++x) {
-                    if (x + 1 < 8) load_w_chunk(x + 1);
-                    asm volatile("" ::: "memory");      // keep the later chunks' loads behind these FMAs
-#pragma unroll
-                    for (int k = 0; k < ITS; ++k) {
-                        const ulonglong2 xv = reinterpret_cast<const ulonglong2*>(Xl + k * kIn)[x];
+                    for (int rel = 0; rel < 2; ++rel)
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
-                            if (x == 0) z0[k][u] = fmul2(xv.x, w[u][0]);                // eq. 1
-                            else ffma2(z0[k][u], xv.x, w[u][2 * x]);
-                            ffma2(z0[k][u], xv.y, w[u][2 * x + 1]);
+                            const int unit = (rel ? lu ^ HL : lu) + u * LPS;
+                            const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(Wh + (c * S + unit) * 4);
+                            w[rel][u][2 * c] = a.x; w[rel][u][2 * c + 1] = a.y;
                         }
-                    }
-                }
+                };
+                mbar_wait(bar_full + 8 * xst, xph);
+                const float* Xh = Xl + 16 * kh;              // this lane's half of its rows
+                load_w_chunk(0);
 #pragma unroll
                 for (int q = 0; q < NSPLIT; ++q) {
                     float pv[ITS];
 #pragma unroll
-                    for (int k = 0; k < ITS; ++k) {
-                        const int it = q * ITS + k;
-                        f32x2 a[4];
-                        if (q == 0) {
+                    for (int k0 = 0; k0 < ITS; k0 += RP) {
+                        f32x2 a[RP][2][4];
 #pragma unroll
-                            for (int u = 0; u < 4; ++u) a[u] = z0[k][u];
-                        } else {
-                            const ulonglong2* xrow = reinterpret_cast<const ulonglong2*>(Xl + it * kIn);
+                        for (int c = 0; c < 4; ++c) {
+                            if (q == 0 && k0 == 0) {
+                                if (c + 1 < 4) load_w_chunk(c + 1);
+                                asm volatile("" ::: "memory");   // keep the later chunks' loads behind these FMAs
+                            }
 #pragma unroll
-                            for (int x = 0; x < 8; ++x) {
-                                const ulonglong2 xv = xrow[x];
+                            for (int r = 0; r < RP; ++r) {
+                                const ulonglong2 xv = reinterpret_cast<const ulonglong2*>(Xh + (q * ITS + k0 + r) * kIn)[c];
 #pragma unroll
-                                for (int u = 0; u < 4; ++u) {
-                                    if (x == 0) a[u] = fmul2(xv.x, w[u][0]);            // eq. 1
-                                    else ffma2(a[u], xv.x, w[u][2 * x]);
-                                    ffma2(a[u], xv.y, w[u][2 * x + 1]);
-                                }
+                                for (int rel = 0; rel < 2; ++rel)
+#pragma unroll
+                                    for (int u = 0; u < 4; ++u) {
+                                        if (c == 0) a[r][rel][u] = fmul2(xv.x, w[rel][u][0]);        // eq. 1
+                                        else ffma2(a[r][rel][u], xv.x, w[rel][u][2 * c]);
+                                        ffma2(a[r][rel][u], xv.y, w[rel][u][2 * c + 1]);
+                                    }
                             }
                         }
 #pragma unroll
-                        for (int u = 0; u < 4; ++u) hreg[it][u] = fmaxf(hsum2(a[u]), 0.f);   // eq. 2
-                        pv[k] = fmaf(hreg[it][1], w2r[1], hreg[it][0] * w2r[0]) +            // eq. 3
-                                fmaf(hreg[it][3], w2r[3], hreg[it][2] * w2r[2]);
+                        for (int r = 0; r < RP; ++r) {
+                            const int it = q * ITS + k0 + r;
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                const float z = hsum2(a[r][0][u]) + __shfl_xor_sync(0xffffffffu, hsum2(a[r][1][u]), pxor);
+                                hreg[it][u] = fmaxf(z, 0.f);                                         // eq. 2
+                            }
+                            pv[k0 + r] = fmaf(hreg[it][1], w2r[1], hreg[it][0] * w2r[0]) +           // eq. 3
+                                         fmaf(hreg[it][3], w2r[3], hreg[it][2] * w2r[2]);
+                        }
                     }
                     GroupReduce<ITS, LPS, 1, LSH>::run(pv, lu);
                     // push: lane l serves ONE destination CTA (pd) and the rows l/C, l/C + 32/C, ...
