@@ -1,14 +1,19 @@
-// eval_tf32.cu -- tensor-core variant of the eval pass (SURVEY.md 8(a) rows a-E / a-T):
+// eval_tc.cu -- tensor-core variants of the eval pass (SURVEY.md 8(a) rows a-E / a-T, 8(f) NEXT-1):
 //   L = (1/n) sum_r (ReLU(X_r W1) W2 - Y_r)^2          (eqs. 1-4)
-// with eq. 1 on the 5th-generation tensor cores (tcgen05.mma kind::tf32: the fp32 operands are
-// read straight from shared memory and truncated to TF32 by the tensor core; fp32 accumulate in
-// TMEM).  Separately reported variant with its own tolerance (loss within 1 % of the oracle,
-// DESIGN.md): it is what makes the pass HBM-bound -- the exact-fp32 kernel is bound by the FP32
-// pipes at 128 FLOP/B.
+// with eq. 1 on the 5th-generation tensor cores (tcgen05.mma, fp32 accumulate in TMEM).  Three operand
+// modes, each a separately reported variant with its own tolerance:
+//   TF32    kind::tf32: the fp32 operands are read straight from shared memory and truncated to TF32 by the
+//           tensor core (loss within 1 % of the oracle; measured <= 4e-4);
+//   BF16    kind::f16 with BF16 operands: four converter warps round the landed X tile to BF16 in place
+//           (round to nearest even), half the tensor time per sample (loss within 1 %; measured <= 1e-4);
+//   TF32X3  three TF32 products X W + (X - trunc X) W + X (W - trunc W): the converter warps write the
+//           residual tile beside the landed one; fp32-faithful (loss within 1e-5).
+// This is what makes the pass HBM-bound -- the exact-fp32 kernel is bound by the FP32 pipes at 128 FLOP/B.
 //
 // Persistent grid, one CTA per SM, warp-specialised:
 //   warp 0      TMA producer: 128-row X tiles (16 KB) by cp.async.bulk.tensor with the 128-byte
 //               swizzle the MMA wants, into a kStages-deep ring;
+//   warps 11-14 (BF16 / TF32X3 only) converters: a thread owns one row of the landed tile;
 //   warp 1, 10  MMA issuers (even / odd tiles): per tile and column part four tcgen05.mma
 //               (M=128, N=hidden/NH, K=8) into the TMEM accumulator of that tile parity
 //               (2 x 256 columns = all of TMEM); tcgen05.commit releases the ring slot and
@@ -31,16 +36,18 @@ namespace {
 constexpr int kTile = 128;           // rows per MMA (M)
 constexpr int kStages = 6;           // X ring depth (6 x 16 KB)
 constexpr int kEvalThreads = 352;    // producer + MMA (even tiles) + 8 epilogue warps + MMA (odd tiles)
+constexpr int kConvThreads = 128;    // converter warps of the BF16 / TF32X3 modes (one thread per tile row)
+enum { kModeTf32 = 0, kModeBf16 = 1, kModeTf32x3 = 2 };
 constexpr uint32_t kTileBytes = kTile * kIn * 4;
 
 // Hidden widths above 256 (one MMA N-extent, half of TMEM) are processed as NS = H/256 column
 // slices per tile: the X tile is read from HBM once, slice sl of a tile goes to accumulator
 // (sl & 1), and the two epilogue sets combine their per-row partial sums through shared memory.
-constexpr int eval_stages(int H) { return H >= 1024 ? 4 : kStages; }
+constexpr int eval_stages(int H, int mode) { return (H >= 1024 || mode == kModeTf32x3) ? 4 : kStages; }
 
-template <int H>
-__global__ void __launch_bounds__(kEvalThreads, 1)
-k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y, long long n,
+template <int H, int MODE>
+__global__ void __launch_bounds__(kEvalThreads + (MODE == kModeTf32 ? 0 : kConvThreads), 1)
+k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y, long long n,
             const float* __restrict__ W1, const float* __restrict__ W2,
             double* __restrict__ partials, unsigned int* __restrict__ ticket,
             double* __restrict__ out) {
@@ -51,23 +58,26 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     // next item's first part overlaps the epilogue of this item's second part.
     constexpr int NH = HS >= 128 ? 2 : 1;
     constexpr int CP = HS / NH;                // columns (hidden units) per part
-    constexpr int NST = eval_stages(H);        // X ring depth
+    constexpr int NST = eval_stages(H, MODE);  // X ring depth
+    constexpr int NB = MODE == kModeTf32x3 ? 2 : 1;       // operand copies (value, residual)
+    static_assert(MODE != kModeTf32x3 || H <= 256, "the three-product mode keeps two copies of both operands");
     constexpr int NG = H / 32;                 // 32-unit groups
     // 1024-byte alignment: swizzle atoms of both operands (checked below)
     extern __shared__ __align__(1024) unsigned char smem[];
-    float* Bs = reinterpret_cast<float*>(smem);                            // [H][32] swizzled
-    unsigned char* Xring = smem + H * kIn * 4;                             // [NST][16 KB]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(Xring + NST * kTileBytes);   // full, empty, tfull[2][NH], tempty[2][NH]
-    double* wsum = reinterpret_cast<double*>(bars + 2 * NST + 16);         // [8]
+    float* Bs = reinterpret_cast<float*>(smem);                            // [NB][H][128 B] swizzled rows (fp32 or bf16)
+    unsigned char* Xring = smem + NB * H * kIn * 4;                        // [NB][NST][16 KB]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(Xring + NB * NST * kTileBytes);   // full, empty, tfull[2][NH], tempty[2][NH], conv
+    double* wsum = reinterpret_cast<double*>(bars + 3 * NST + 16);         // [8]
     float* rowpart = reinterpret_cast<float*>(wsum + 8);                   // [2][128] partial rows of set 1
     int* wcnt = reinterpret_cast<int*>(rowpart + 2 * kTile);               // [32]
     int* npos_s = wcnt + 32;
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(npos_s + 1);
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + NST),
-                   bar_tfull = smem_u32(bars + 2 * NST), bar_tempty = smem_u32(bars + 2 * NST + 8);
+                   bar_tfull = smem_u32(bars + 2 * NST), bar_tempty = smem_u32(bars + 2 * NST + 8),
+                   bar_conv = smem_u32(bars + 2 * NST + 16);               // [NST] tile converted (BF16 / TF32X3)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NW = kEvalThreads / 32;
+    constexpr int NW = (kEvalThreads + (MODE == kModeTf32 ? 0 : kConvThreads)) / 32;
     __shared__ int last_flag_s;
     int* last_flag = &last_flag_s;
 
@@ -80,7 +90,10 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
     // is summed with +-1 weights kept in registers.  Columns 24..31 of every chunk take ReLU as
     // (z + |z|) on the FMA pipe and carry a factor 1/2.
     if (tid == 0) {
-        for (int s = 0; s < NST; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NS > 1 ? 2 : 1); }
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NS > 1 ? 2 : 1);
+            mbar_init(bar_conv + 8 * s, kConvThreads / 32);
+        }
         for (int b = 0; b < 8; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
         fence_mbar_init();
     }
@@ -122,9 +135,28 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
         if (j0 == 0) *npos_s = total;
         unsigned char* brow = smem + (j >> 3) * 1024 + (j & 7) * 128;    // K-major row, 128B swizzle
 #pragma unroll
-        for (int c = 0; c < kIn / 4; ++c)
-            *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
-                make_float4(wcol[4 * c] * sc, wcol[4 * c + 1] * sc, wcol[4 * c + 2] * sc, wcol[4 * c + 3] * sc);
+        for (int k = 0; k < kIn; ++k) wcol[k] *= sc;
+        if constexpr (MODE == kModeBf16) {                               // 32 bf16 = the first 64 logical bytes of the row
+#pragma unroll
+            for (int c = 0; c < kIn / 8; ++c)
+                *reinterpret_cast<uint4*>(brow + ((c ^ (j & 7)) << 4)) =
+                    make_uint4(bf16x2(wcol[8 * c], wcol[8 * c + 1]), bf16x2(wcol[8 * c + 2], wcol[8 * c + 3]),
+                               bf16x2(wcol[8 * c + 4], wcol[8 * c + 5]), bf16x2(wcol[8 * c + 6], wcol[8 * c + 7]));
+        } else {
+#pragma unroll
+            for (int c = 0; c < kIn / 4; ++c) {
+                if constexpr (MODE == kModeTf32x3)                       // value operand already exact in TF32
+                    *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
+                        make_float4(tf32_trunc(wcol[4 * c]), tf32_trunc(wcol[4 * c + 1]), tf32_trunc(wcol[4 * c + 2]), tf32_trunc(wcol[4 * c + 3]));
+                else
+                    *reinterpret_cast<float4*>(brow + ((c ^ (j & 7)) << 4)) =
+                        make_float4(wcol[4 * c], wcol[4 * c + 1], wcol[4 * c + 2], wcol[4 * c + 3]);
+                if constexpr (MODE == kModeTf32x3)                       // what the truncation drops (exact in fp32)
+                    *reinterpret_cast<float4*>(brow + H * 128 + ((c ^ (j & 7)) << 4)) =
+                        make_float4(tf32_residual(wcol[4 * c]), tf32_residual(wcol[4 * c + 1]),
+                                    tf32_residual(wcol[4 * c + 2]), tf32_residual(wcol[4 * c + 3]));
+            }
+        }
     }
     if (warp == 1) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot))
@@ -162,30 +194,76 @@ k_eval_tf32(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__
         // that neither epilogue set ever waits behind the other set's TMEM hand-back (whole warp runs
         // the loop, one elected lane issues) =====
         // instruction descriptor: D=f32, A=B=tf32, both K-major, N=CP, M=128
-        constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(CP >> 3) << 17) |
-                                   ((uint32_t)(kTile >> 4) << 24);
+        constexpr uint32_t idesc = mma_idesc(MODE == kModeBf16 ? 1u : 2u, kTile, CP);
         const uint64_t bdesc = smem_desc_sw128(smem_u32(Bs));
         const uint64_t adesc0 = smem_desc_sw128(smem_u32(Xring));
         const uint32_t b = warp == 1 ? 0u : 1u;
         for (uint32_t w = b, kth = 0; w < nitems; w += 2, ++kth) {
             const uint32_t i = w / NS, sl = w % NS, st = i % NST;
             const uint32_t tph = (kth - 1u) & 1u;
-            mbar_wait(bar_full + 8 * st, (i / NST) & 1u);
+            mbar_wait((MODE == kModeTf32 ? bar_full : bar_conv) + 8 * st, (i / NST) & 1u);
             const uint64_t adesc = adesc0 + (uint64_t)(st * (kTileBytes >> 4));
 #pragma unroll
             for (int hf = 0; hf < NH; ++hf) {
                 if (kth >= 1) mbar_wait(bar_tempty + 8 * (NH * b + hf), tph);
                 tc_fence_after();
                 if (elect_one()) {
+                    const uint32_t dcol = tmem_base + b * 256 + hf * CP;
+                    const uint64_t bd = bdesc + (uint64_t)((sl * HS + hf * CP) * 128 / 16);
+                    if constexpr (MODE == kModeBf16) {
 #pragma unroll
-                    for (int k = 0; k < kIn / 8; ++k)  // K = 8 tf32 = 32 bytes per MMA: +2 in 16-byte units
-                        mma_tf32(tmem_base + b * 256 + hf * CP, adesc + 2 * k,
-                                 bdesc + (uint64_t)((sl * HS + hf * CP) * 128 / 16) + 2 * k, idesc, k > 0);
+                        for (int k = 0; k < kIn / 16; ++k)  // K = 16 bf16 = 32 bytes per MMA: +2 in 16-byte units
+                            mma_f16(dcol, adesc + 2 * k, bd + 2 * k, idesc, k > 0);
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < kIn / 8; ++k)   // K = 8 tf32 = 32 bytes per MMA: +2 in 16-byte units
+                            mma_tf32(dcol, adesc + 2 * k, bd + 2 * k, idesc, k > 0);
+                        if constexpr (MODE == kModeTf32x3) {
+                            constexpr uint64_t xl = (uint64_t)(NST * kTileBytes >> 4), bl = (uint64_t)(H * 128 >> 4);
+#pragma unroll
+                            for (int k = 0; k < kIn / 8; ++k)   // + (X - trunc X) trunc W
+                                mma_tf32(dcol, adesc + xl + 2 * k, bd + 2 * k, idesc, 1u);
+#pragma unroll
+                            for (int k = 0; k < kIn / 8; ++k)   // + trunc X (W - trunc W)
+                                mma_tf32(dcol, adesc + 2 * k, bd + bl + 2 * k, idesc, 1u);
+                        }
+                    }
                     // ring slot free once the last slice this issuer takes from the tile has read it
                     if (hf == NH - 1 && sl + 2 >= NS) tc_commit(bar_empty + 8 * st);
                     tc_commit(bar_tfull + 8 * (NH * b + hf));           // accumulator part ready
                 }
                 __syncwarp();
+            }
+        }
+    } else if (warp >= kEvalThreads / 32) {
+        // ===== converters (BF16 / TF32X3): a thread owns one row of every landed tile =====
+        if constexpr (MODE != kModeTf32) {
+            const int r = tid - kEvalThreads;                                   // tile row 0..127
+            for (uint32_t i = 0; i < nt; ++i) {
+                const uint32_t st = i % NST;
+                mbar_wait(bar_full + 8 * st, (i / NST) & 1u);
+                unsigned char* row = Xring + st * kTileBytes + r * 128;
+                float4 v[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) v[c] = *reinterpret_cast<const float4*>(row + ((c ^ (r & 7)) << 4));
+                if constexpr (MODE == kModeBf16) {                              // in place: 32 bf16 in the first 64 logical bytes
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+                        *reinterpret_cast<uint4*>(row + ((c ^ (r & 7)) << 4)) =
+                            make_uint4(bf16x2(v[2 * c].x, v[2 * c].y), bf16x2(v[2 * c].z, v[2 * c].w),
+                                       bf16x2(v[2 * c + 1].x, v[2 * c + 1].y), bf16x2(v[2 * c + 1].z, v[2 * c + 1].w));
+                } else {                                                        // value exact in TF32 in place, residual beside it
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        *reinterpret_cast<float4*>(row + ((c ^ (r & 7)) << 4)) =
+                            make_float4(tf32_trunc(v[c].x), tf32_trunc(v[c].y), tf32_trunc(v[c].z), tf32_trunc(v[c].w));
+                        *reinterpret_cast<float4*>(row + NST * kTileBytes + ((c ^ (r & 7)) << 4)) =
+                            make_float4(tf32_residual(v[c].x), tf32_residual(v[c].y), tf32_residual(v[c].z), tf32_residual(v[c].w));
+                    }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes -> MMA (async proxy)
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_conv + 8 * st);
             }
         }
     } else {
@@ -319,16 +397,27 @@ EncodeTiledFn encode_tiled() {
     return fn;
 }
 
-template <int H>
-cudaError_t launch_h(const CUtensorMap& tmap, const float* Y, long long n, const float* W1, const float* W2,
-                     double* partials, unsigned int* ticket, int grid, double* d_out, cudaStream_t stream) {
-    auto kern = k_eval_tf32<H>;
-    const size_t smem = (size_t)H * kIn * 4 + (size_t)eval_stages(H) * kTileBytes + (size_t)H * 4 + 2 * kTile * 4 + 32 * 4 +
-                        8 * (2 * kStages + 16) + 8 * 8 + 4 * H + 32 + 4 + 16;
+template <int H, int MODE>
+cudaError_t launch_hm(const CUtensorMap& tmap, const float* Y, long long n, const float* W1, const float* W2,
+                      double* partials, unsigned int* ticket, int grid, double* d_out, cudaStream_t stream) {
+    auto kern = k_eval_tc<H, MODE>;
+    constexpr int NB = MODE == kModeTf32x3 ? 2 : 1;
+    constexpr int NST = eval_stages(H, MODE);
+    const size_t smem = (size_t)NB * H * kIn * 4 + (size_t)NB * NST * kTileBytes + 8 * (3 * NST + 16) + 8 * 8 + 2 * kTile * 4 +
+                        32 * 4 + 4 + 4 + 64;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
-    kern<<<grid, kEvalThreads, smem, stream>>>(tmap, Y, n, W1, W2, partials, ticket, d_out);
+    kern<<<grid, kEvalThreads + (MODE == kModeTf32 ? 0 : kConvThreads), smem, stream>>>(tmap, Y, n, W1, W2, partials, ticket, d_out);
     return cudaGetLastError();
+}
+
+template <int H>
+cudaError_t launch_h(int mode, const CUtensorMap& tmap, const float* Y, long long n, const float* W1, const float* W2,
+                     double* partials, unsigned int* ticket, int grid, double* d_out, cudaStream_t stream) {
+    if (mode == kModeBf16) return launch_hm<H, kModeBf16>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream);
+    if constexpr (H <= 256)
+        if (mode == kModeTf32x3) return launch_hm<H, kModeTf32x3>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream);
+    return launch_hm<H, kModeTf32>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream);
 }
 
 }  // namespace
@@ -345,9 +434,12 @@ bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows) {
                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// variant numbers of include/mlp.h: 2 = MLP_VARIANT_TF32, 5 = MLP_VARIANT_BF16, 6 = MLP_VARIANT_TF32X3
 bool eval_tc_supported(int hidden, int variant) {
-    if (variant != 2 /* MLP_VARIANT_TF32 */) return false;
-    return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256 || hidden == 512 || hidden == 1024;
+    const bool width = hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256 || hidden == 512 || hidden == 1024;
+    if (variant == 2 || variant == 5) return width;
+    if (variant == 6) return width && hidden <= 256;
+    return false;
 }
 
 cudaError_t launch_eval_tc(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
@@ -355,18 +447,19 @@ cudaError_t launch_eval_tc(const float* X, const float* Y, int64_t n, const floa
                            cudaStream_t stream, int64_t* launches) {
     if (!eval_tc_supported(hidden, variant)) return cudaErrorInvalidValue;
     if (n > 0x7fffffffLL - kTile) return cudaErrorInvalidValue;      // TMA coordinates are int32
+    const int mode = variant == 5 ? kModeBf16 : variant == 6 ? kModeTf32x3 : kModeTf32;
     // X as a 2-D tensor [n rows][32 floats]; box = one 128-row tile; 128-byte swizzle = the layout
     // tcgen05.mma reads a K-major operand in (a row is exactly one 128-byte swizzle span).
     CUtensorMap tmap;
     if (!make_x_tensormap(&tmap, X, n, kTile)) return cudaErrorNotSupported;
     cudaError_t err;
     switch (hidden) {
-        case 32: err = launch_h<32>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
-        case 64: err = launch_h<64>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
-        case 128: err = launch_h<128>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
-        case 256: err = launch_h<256>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
-        case 512: err = launch_h<512>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
-        case 1024: err = launch_h<1024>(tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 32: err = launch_h<32>(mode, tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 64: err = launch_h<64>(mode, tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 128: err = launch_h<128>(mode, tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 256: err = launch_h<256>(mode, tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 512: err = launch_h<512>(mode, tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
+        case 1024: err = launch_h<1024>(mode, tmap, Y, n, W1, W2, partials, ticket, grid, d_out, stream); break;
         default: return cudaErrorInvalidValue;
     }
     if (err == cudaSuccess) ++*launches;

@@ -68,6 +68,9 @@ __device__ __forceinline__ uint32_t bf16x2(float lo, float hi) {
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
+// fp32 -> the TF32 value the tensor core would use (low 13 mantissa bits dropped), and what that drops (exact in fp32)
+__device__ __forceinline__ float tf32_trunc(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+__device__ __forceinline__ float tf32_residual(float x) { return x - tf32_trunc(x); }
 // instruction descriptor of tcgen05.mma: fp32 accumulate, both operands K-major, A/B format `fmt`
 // (kind::tf32: 2 = TF32; kind::f16: 1 = BF16), N and M extents
 __host__ __device__ constexpr uint32_t mma_idesc(uint32_t fmt, int M, int N) {

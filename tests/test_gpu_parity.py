@@ -317,6 +317,54 @@ def test_eval_tf32_sign_layouts(hidden, npos):
     assert abs(lg - lo) <= 5e-3 * lo, (hidden, npos, lg, lo)
 
 
+# BF16 operands (converted in the kernel, round to nearest even), fp32 accumulate: stated tolerance = loss within
+# 1 % of the oracle (eval-only quantisation error 7e-5 at survey time).
+@pytest.mark.parametrize("hidden", [32, 64, 128, 256, 512, 1024])
+@pytest.mark.parametrize("n", [1, 127, 128, 5000, 70001, 300000])
+def test_eval_bf16_variant(hidden, n):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(5, 32, hidden)
+    lg, lo = gpu_eval(X, Y, W1, W2, variant=B.VARIANT_BF16), O.eval_loss(X, Y, W1, W2)
+    assert abs(lg - lo) <= 1e-2 * lo, (hidden, n, lg, lo)
+    assert abs(lg - lo) <= 5e-3 * lo, ("bf16 error larger than expected", hidden, n, lg, lo)
+    assert gpu_eval(X, Y, W1, W2, variant=B.VARIANT_BF16) == lg      # deterministic
+
+
+# Three TF32 products (value x value + residual x value + value x residual): fp32-faithful, stated tolerance 1e-5
+# on the loss; hidden <= 256.
+@pytest.mark.parametrize("hidden", [32, 64, 128, 256])
+@pytest.mark.parametrize("n", [1, 127, 128, 5000, 70001, 300000])
+def test_eval_tf32x3_variant(hidden, n):
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(5, 32, hidden)
+    lg, lo = gpu_eval(X, Y, W1, W2, variant=B.VARIANT_TF32X3), O.eval_loss(X, Y, W1, W2)
+    assert abs(lg - lo) <= 1e-5 * lo, (hidden, n, lg, lo)
+    assert gpu_eval(X, Y, W1, W2, variant=B.VARIANT_TF32X3) == lg    # deterministic
+
+
+def test_eval_tf32x3_unsupported_width():
+    X, Y = datagen.make_dataset(1000, 0.1)
+    W1, W2 = O.init_weights(5, 32, 512)
+    with pytest.raises(B.MlpError) as e:
+        gpu_eval(X, Y, W1, W2, variant=B.VARIANT_TF32X3)
+    assert e.value.code == 3
+
+
+@pytest.mark.parametrize("variant", ["bf16", "tf32x3"])
+@pytest.mark.parametrize("npos", ["all", "none", 1, 31, 32, 33, 255])
+def test_eval_tc_modes_sign_layouts(variant, npos):
+    hidden, n = 256, 3000
+    X, Y = datagen.make_dataset(n, 0.1)
+    W1, W2 = O.init_weights(7, 32, hidden)
+    W2 = np.abs(W2) + np.float32(1e-3)
+    k = hidden if npos == "all" else 0 if npos == "none" else min(int(npos), hidden)
+    neg = np.random.default_rng(11).permutation(hidden)[k:]
+    W2[neg] = -W2[neg]
+    v, tol = (B.VARIANT_BF16, 5e-3) if variant == "bf16" else (B.VARIANT_TF32X3, 1e-5)
+    lg, lo = gpu_eval(X, Y, W1, W2, variant=v), O.eval_loss(X, Y, W1, W2)
+    assert abs(lg - lo) <= tol * lo, (variant, npos, lg, lo)
+
+
 def test_eval_closed_forms():
     X, Y = datagen.make_dataset(50000, 0.1)
     W1, _ = O.init_weights(5, 32, 256)
