@@ -1,27 +1,29 @@
-// train_tf32.cu -- tensor-core variant of the fused training kernel (SURVEY.md 8(a) row a-T,
-// 8(f) NEXT-2; BASELINE.json: "allowed only as a separately reported variant with its own stated
-// tolerance").  Same method, same loop, same cluster layout and Ypred exchange as train_fused.cu
-// (eqs. 1-9; one launch for every batch of every epoch), but both large products
-// run on the tensor cores (tcgen05.mma kind::tf32: fp32 operands truncated to TF32, fp32
-// accumulate in TMEM):
-//   eq. 1  Z1 = X W1        per 256-row tile two chains M=128 (rows), N=32 (units of this CTA), K=32;
-//   eq. 8  dW1^T = dZ1^T X  one chain M=64 (32 units + padding), N=32 (inputs), K=256 rows, in TMEM
-//                           across the tiles of a batch.
-// Everything else stays fp32 on the CUDA cores.  32 hidden units per CTA: hidden 32..256 on a
-// cluster of hidden/32 CTAs (the exchange buffers of a 16-CTA cluster no longer fit beside the
-// operands of eq. 8 in shared memory; hidden 1024 would need 32 CTAs per cluster).
+// train_tc.cu -- tensor-core variants of the fused training kernel (SURVEY.md 8(a) row a-T, 8(f) NEXT-2;
+// BASELINE.json: "allowed only as a separately reported variant with its own stated tolerance").
+// Same method, same loop, same cluster layout and Ypred exchange as train_fused.cu (eqs. 1-9,
+// PAPER.md:44-71; one launch for every batch of every epoch), but both large products run on the
+// tensor cores (tcgen05.mma, fp32 accumulate in TMEM, fp32 master weights):
+//   eq. 1  Z1 = X W1        per tile chains of M=128 (rows), N=32 or 64 (units of this CTA), K=32;
+//   eq. 8  dW1^T = dZ1^T X  one chain M=64 (units), N=32 (inputs), K = rows of the tile, accumulated in
+//                           TMEM across the tiles of a batch.
+// Operand precision: TF32 (kind::tf32: fp32 bits in shared memory, truncated by the tensor core) or BF16
+// (kind::f16: the threads round every operand to BF16, round to nearest even, as they stage it).
+// Everything else stays fp32 on the CUDA cores.
 //
-// Per tile and CTA (8 warps, a thread owns ONE row of the tile):
-//   TMA (cp.async.bulk.tensor, 128-byte swizzle) brings the X tile [256 x 32] one tile ahead; warp 0
-//   issues eq. 1 (A = X tile as delivered, B = W1^T slice in operand layout); while it runs every thread
-//   transposes its X row into the K-major B operand of eq. 8; then it reads its 32 pre-activations
-//   from TMEM, applies eq. 2, stores H, forms its partial of eq. 3 and pushes it to the 8 CTAs
-//   (st.async + mbarrier); after the exchange it computes dZ2 (eq. 5) and writes its row of
-//   dZ1 = dZ2 ReLU'(Z1) W2 (eq. 7) into the K-major A operand of eq. 8; warp 0 issues eq. 8 while all
-//   warps do eq. 6 (dW2) on the CUDA cores.  At the end of the batch the 32 threads that own the TMEM
-//   rows of dW1^T (one per hidden unit) apply eq. 9 to the fp32 master row they keep in registers and
-//   rewrite their row of the eq. 1 operand.  No W1 register reload, no CUDA-core backward loop.
-// All operands are K-major with the 128-byte swizzle (the conventions of eval_tf32.cu).
+// Two geometries (template parameter S = hidden units per CTA):
+//   S = 32: 256-row tiles, a thread owns ONE row;        hidden 32..256  on clusters of 1..8 CTAs,
+//   S = 64: 128-row tiles, TWO threads share a row (32 units each); hidden 512, 1024 on clusters of 8, 16.
+//
+// Per tile and CTA (8 warps):
+//   TMA (cp.async.bulk.tensor, 128-byte swizzle) brings the X tile one tile ahead; warp 0 issues eq. 1
+//   (A = X tile, B = W1^T slice in operand layout); meanwhile every thread transposes its part of its X
+//   row into the K-major B operand of eq. 8; then it reads its 32 pre-activations from TMEM, applies
+//   eq. 2, stores H, forms its partial of eq. 3 and pushes it to every CTA of the cluster (st.async +
+//   mbarrier); after the exchange it computes dZ2 (eq. 5) and writes its part of dZ1 = dZ2 ReLU'(Z1) W2
+//   (eq. 7) into the K-major A operand of eq. 8; warp 0 issues eq. 8 while all warps do eq. 6 (dW2) on
+//   the CUDA cores.  At the end of the batch the threads that own the TMEM rows of dW1^T (one per hidden
+//   unit) apply eq. 9 to the fp32 master row they keep in registers and rewrite their row of the eq. 1
+//   operand.  All operands are K-major with the 128-byte swizzle (the conventions of eval_tc.cu).
 #include <cuda.h>
 
 #include "tc_common.cuh"
@@ -29,13 +31,9 @@
 namespace mlp {
 namespace {
 
-constexpr int kS = 32;            // hidden units per CTA
-// cluster size C = hidden / 32 is a template parameter (1, 2, 4 or 8)
-constexpr int kBT = 256;          // rows per tile
 constexpr int kWarps = 8;
 constexpr int kThreads = kWarps * 32;
-constexpr int kRing = 2;          // X ring stages (the operands of eq. 8 take the rest of shared memory)
-constexpr uint32_t kXBytes = kBT * kIn * 4;
+constexpr int kRing = 2;          // X ring stages
 
 struct TcParams {
     const float* Y;
@@ -52,23 +50,60 @@ struct TcParams {
     unsigned long long* stats;   // [4] = batch_order entries outside [0, nb) (clamped and counted)
 };
 
-template <int C>
+// shared-memory plan, shared by the kernel and its launcher
+template <int C, int S, bool BF16>
+struct TcPlan {
+    static constexpr int NTH = S / 32;                 // threads per row
+    static constexpr int BT = 256 / NTH;               // rows per tile
+    static constexpr int EB = BF16 ? 2 : 4;            // operand element bytes
+    static constexpr int KA = 128 / EB;                // rows (K elements) per 128-byte swizzle atom of eq. 8
+    static constexpr int NA = BT / KA;                 // K atoms of eq. 8
+    static constexpr int NSL = C * NTH;                // Ypred partial slots per row
+    static constexpr uint32_t XBYTES = BT * 128;       // one X tile
+    static constexpr uint32_t oX = 0;                                   // [kRing][BT][128 B]  A of eq. 1 (TF32)
+    static constexpr uint32_t oXb = oX + kRing * XBYTES;                // [BT][128 B]         A of eq. 1 (BF16 copy)
+    static constexpr uint32_t oW = oXb + (BF16 ? XBYTES : 0);           // [S][128 B]          B of eq. 1
+    static constexpr uint32_t oAt = oW + S * 128;                       // [NA][64][128 B]     A of eq. 8 (dZ1^T)
+    static constexpr uint32_t oXt = oAt + NA * 64 * 128;                // [NA][32][128 B]     B of eq. 8 (X^T)
+    static constexpr uint32_t oH = oXt + NA * 32 * 128;                 // [NTH][BT][128 B]    H = ReLU(Z1)
+    static constexpr uint32_t oYp = oH + NTH * BT * 128;                // [2][NSL][BT] floats
+    static constexpr uint32_t oP2 = oYp + 2 * NSL * BT * 4;             // [kWarps][32] dW2 partials
+    static constexpr uint32_t oW2 = oP2 + kWarps * 32 * 4;              // [S]
+    static constexpr uint32_t oD = oW2 + S * 4;                         // [BT] dZ2 of the tile
+    static constexpr uint32_t oBar = (oD + BT * 4 + 7) / 8 * 8;         // full[kRing], empty[kRing], yp[2], mma, mma2
+    static constexpr uint32_t oTm = oBar + 8 * (2 * kRing + 4);
+    static constexpr uint32_t BYTES = oTm + 16;
+};
+
+// 8 floats -> 8 packed bf16 (16 bytes)
+__device__ __forceinline__ uint4 pack_bf16x8(const float* v) {
+    return make_uint4(bf16x2(v[0], v[1]), bf16x2(v[2], v[3]), bf16x2(v[4], v[5]), bf16x2(v[6], v[7]));
+}
+__device__ __forceinline__ unsigned short bf16_bits(float v) {
+    unsigned short r;
+    asm("cvt.rn.bf16.f32 %0, %1;" : "=h"(r) : "f"(v));
+    return r;
+}
+
+template <int C, int S, bool BF16>
 __global__ void __launch_bounds__(kThreads, 1)
-k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
-    constexpr int S = kS, BT = kBT;
-    constexpr int NA = BT / 32;                                           // 32-row K atoms of the backward product
+k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
+    using P = TcPlan<C, S, BF16>;
+    constexpr int NTH = P::NTH, BT = P::BT, NA = P::NA, NSL = P::NSL;
+    constexpr uint32_t kXBytes = P::XBYTES;
     extern __shared__ __align__(1024) unsigned char smem[];
-    unsigned char* Xs = smem;                                             // [kRing][32 KB] X tiles, swizzled rows (A of eq. 1)
-    unsigned char* Wop = Xs + kRing * kXBytes;                            // [S][128 B] W1^T slice (B of eq. 1), K-major swizzled
-    unsigned char* At = Wop + S * 128;                                    // [NA][64][128 B] dZ1^T (A of eq. 8), rows 32-63 padding
-    unsigned char* Xt = At + NA * 64 * 128;                               // [NA][32][128 B] X^T (B of eq. 8)
-    unsigned char* Hs = Xt + NA * 32 * 128;                               // [BT][128 B] H = ReLU(Z1), swizzled rows (eq. 6)
-    float* ypp = reinterpret_cast<float*>(Hs + BT * 128);                 // [2][C][BT]
-    float* part2 = ypp + 2 * C * BT;                                      // [kWarps][S] dW2 partials
-    float* W2s = part2 + kWarps * S;                                      // [S]
-    float* Ds = W2s + S;                                                  // [BT] dZ2 of the tile
-    uint64_t* bars = reinterpret_cast<uint64_t*>(Ds + BT);                // full[3], empty[3], yp[2], mma, mma2
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kRing + 4);
+    unsigned char* Xs = smem + P::oX;
+    unsigned char* Xb = smem + P::oXb;
+    unsigned char* Wop = smem + P::oW;
+    unsigned char* At = smem + P::oAt;
+    unsigned char* Xt = smem + P::oXt;
+    unsigned char* Hs = smem + P::oH;
+    float* ypp = reinterpret_cast<float*>(smem + P::oYp);
+    float* part2 = reinterpret_cast<float*>(smem + P::oP2);
+    float* W2s = reinterpret_cast<float*>(smem + P::oW2);
+    float* Ds = reinterpret_cast<float*>(smem + P::oD);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P::oBar);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + P::oTm);
     const uint32_t bar_full = smem_u32(bars), bar_empty = smem_u32(bars + kRing),
                    bar_yp = smem_u32(bars + 2 * kRing), bar_mma = smem_u32(bars + 2 * kRing + 2),
                    bar_mma2 = smem_u32(bars + 2 * kRing + 3);
@@ -76,19 +111,27 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t crank = cluster_ctarank();
     const int H = p.H;
-    // forward ownership: thread <-> tile row (TMEM lane rule: warp w reads lanes 32*(w%4)..)
-    const int frow = (warp >> 2) * 128 + (warp & 3) * 32 + lane;
+    // thread <-> (tile row, 32-unit half); TMEM lane rule: warp w reads lanes 32*(w%4)..
+    const int blk = warp >> 2, wq = warp & 3;
+    const int frow = (NTH == 1 ? blk * 128 : 0) + wq * 32 + lane;
+    const int hb = NTH == 2 ? blk : 0;                                    // which 32 of the CTA's S units
+    const int uoff = hb * 32;
     // weight ownership: the M=64 accumulator of eq. 8 keeps unit u in TMEM lane (u/16)*32 + u%16, i.e. lanes
-    // 0-15 of warps 0 and 1: those 32 threads hold the fp32 master row W1[:, u] in registers for the whole run
-    const bool wowner = warp < 2 && lane < 16;
+    // 0-15 of warps 0..S/16-1: those threads hold the fp32 master row W1[:, u] in registers for the whole run
+    const bool wowner = warp < S / 16 && lane < 16;
     const int wu = warp * 16 + lane;                                      // owned hidden unit (if wowner)
     float wrow[kIn];
 #pragma unroll
     for (int i = 0; i < kIn; ++i) wrow[i] = wowner ? p.W1[(size_t)i * H + crank * S + wu] : 0.f;
     auto store_wop = [&]() {                                              // B[n = u][k = i], eq. 1 operand
+        if constexpr (BF16) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c)
-            *reinterpret_cast<float4*>(Wop + swz(wu, c)) = make_float4(wrow[4 * c], wrow[4 * c + 1], wrow[4 * c + 2], wrow[4 * c + 3]);
+            for (int c = 0; c < 4; ++c) *reinterpret_cast<uint4*>(Wop + swz(wu, c)) = pack_bf16x8(wrow + 8 * c);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                *reinterpret_cast<float4*>(Wop + swz(wu, c)) = make_float4(wrow[4 * c], wrow[4 * c + 1], wrow[4 * c + 2], wrow[4 * c + 3]);
+        }
     };
 
     // ---- one-time setup ---------------------------------------------------------------------------
@@ -123,7 +166,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
         return t < 0 ? 0 : p.nbi - 1;
     };
     auto rows_of = [&](int t) -> int { return t == p.nbi - 1 ? p.m_last : p.B; };
-    auto issue_tile = [&](long long g0, unsigned nbuf) {      // one thread; the box is always 256 rows
+    auto issue_tile = [&](long long g0, unsigned nbuf) {      // one thread; the box is always BT rows
         mbar_arrive_expect_tx(bar_full + 8 * nbuf, kXBytes);  // rows past n are zero-filled, still counted
         tma_load_2d(smem_u32(Xs) + nbuf * kXBytes, &tmapX, 0, (int)g0, bar_full + 8 * nbuf);
     };
@@ -132,20 +175,27 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     seq = 2 % p.nbi;
     if (tid == 0) issue_tile((long long)t_cur * p.B, 0);
 
-    const uint32_t taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (warp >> 2) * 32;   // eq. 1 accumulators: columns 0-63
-    const uint32_t tdw = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + 64;                   // eq. 8 accumulator: columns 64-95
+    const uint32_t taddr = tmem_base + ((uint32_t)(wq * 32) << 16) + blk * 32;   // eq. 1 accumulators: columns 0-63
+    const uint32_t tdw = tmem_base + ((uint32_t)(wq * 32) << 16) + 64;           // eq. 8 accumulator: columns 64-95
     float ycur = 0.f;
     {
         const long long r0 = (long long)t_cur * p.B;
         if (frow < min(BT, rows_of(t_cur))) ycur = __ldg(p.Y + r0 + frow);
     }
     const uint32_t ypp_a = smem_u32(ypp), yp_a = bar_yp;
-    // instruction descriptors: D=f32, A=B=tf32, both K-major; eq. 1: M=128, N=32; eq. 8: M=64, N=32
-    constexpr uint32_t idesc1 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(S >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-    constexpr uint32_t idesc8 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kIn >> 3) << 17) | ((uint32_t)(64 >> 4) << 24);
-    // position of (row r of the tile, column c) in the K-major operands of eq. 8: atom r/32, operand row c,
-    // k = r%32 inside the 128-byte swizzled row
-    const int ka = frow >> 5, kk = frow & 31;
+    // instruction descriptors: D=f32, both operands K-major; eq. 1: M=128, N=32 (two chains) or 64; eq. 8: M=64, N=32
+    constexpr uint32_t kFmt = BF16 ? 1u : 2u;
+    constexpr uint32_t idesc1 = mma_idesc(kFmt, 128, S == 32 ? 32 : 64);
+    constexpr uint32_t idesc8 = mma_idesc(kFmt, 64, kIn);
+    constexpr int KS1 = BF16 ? 2 : 4;                          // MMAs per chain of eq. 1 (K = 16 or 8 each)
+    // position of (row r of the tile, operand row c) in the K-major operands of eq. 8: atom r/KA, k = r%KA
+    const int ka = BF16 ? frow >> 6 : frow >> 5, kk = BF16 ? frow & 63 : frow & 31;
+    auto t8 = [&](unsigned char* base, int orow, int rows_per_atom) -> unsigned char* {   // address of element (orow, k = frow)
+        return BF16 ? base + ka * (rows_per_atom * 128) + swz(orow, kk >> 3) + (kk & 7) * 2
+                    : base + ka * (rows_per_atom * 128) + swz(orow, kk >> 2) + (kk & 3) * 4;
+    };
+    constexpr int NCH = 8 / NTH;                               // 16-byte chunks of an X row this thread handles
+    const int c0 = NTH == 2 ? hb * 4 : 0;
     unsigned gt = 0;
     for (long long step = 0; step < total; ++step) {
         const int t_nn = (step + 2 < total) ? batch_index(step + 2, seq) : 0;
@@ -154,7 +204,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
         const int m = rows_of(t_cur);
         const int ntiles = (m + BT - 1) / BT;
         const float scale = t_cur == p.nbi - 1 ? p.scale_last : p.scale_full;   // eq. 5: 2 / m
-        float g2 = 0.f;                                        // dW2 partial: unit lane, rows 32*warp.. of every tile
+        float g2 = 0.f;                                        // dW2 partial of one unit over 32 rows of every tile
 
         for (int j = 0; j < ntiles; ++j, ++gt) {
             const unsigned buf = gt & 1u, ph = (gt >> 1) & 1u;
@@ -165,7 +215,7 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
             else if (step + 1 < total) { nr0 = (long long)t_next * p.B; nrows = min(BT, rows_of(t_next)); }
             if (warp == 0) {                                   // converged warp, one elected lane (uniform-register forms)
                 if (elect_one()) {
-                    mbar_arrive_expect_tx(bar_yp + 8 * buf, C * BT * 4);    // arm this tile's exchange
+                    mbar_arrive_expect_tx(bar_yp + 8 * buf, NSL * BT * 4);  // arm this tile's exchange
                     if (nrows > 0) {
                         const unsigned g1 = gt + 1, nbuf = g1 % kRing;
                         if (g1 >= kRing) mbar_wait(bar_empty + 8 * nbuf, ((g1 / kRing) - 1) & 1u);
@@ -179,39 +229,54 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
             // ---------------- eq. 1 on the tensor cores ----------------
             mbar_wait(bar_full + 8 * xst, xph);
-            const unsigned char* Xt_tile = Xs + xst * kXBytes;
-            if (warp == 0) {
-                tc_fence_after();
-                if (elect_one()) {
-                    const uint64_t bdesc = smem_desc_sw128(smem_u32(Wop));
+            const unsigned char* Xtile = Xs + xst * kXBytes;
+            auto issue_eq1 = [&]() {
+                if (warp == 0) {
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint64_t bdesc = smem_desc_sw128(smem_u32(Wop));
 #pragma unroll
-                    for (int a = 0; a < 2; ++a) {              // rows 0-127 / 128-255 of the tile
-                        const uint64_t adesc = smem_desc_sw128(smem_u32(Xs) + xst * kXBytes + a * 128 * 128);
+                        for (int a = 0; a < (NTH == 1 ? 2 : 1); ++a) {     // row blocks of 128 (S = 32: two of them)
+                            const uint64_t adesc = smem_desc_sw128((BF16 ? smem_u32(Xb) : smem_u32(Xs) + xst * kXBytes) + a * 128 * 128);
 #pragma unroll
-                        for (int k = 0; k < kIn / 8; ++k)
-                            mma_tf32(tmem_base + a * 32, adesc + 2 * k, bdesc + 2 * k, idesc1, k > 0);
+                            for (int k = 0; k < KS1; ++k) {
+                                if constexpr (BF16) mma_f16(tmem_base + a * 32, adesc + 2 * k, bdesc + 2 * k, idesc1, k > 0);
+                                else mma_tf32(tmem_base + a * 32, adesc + 2 * k, bdesc + 2 * k, idesc1, k > 0);
+                            }
+                        }
+                        tc_commit(bar_mma);
                     }
-                    tc_commit(bar_mma);
+                    __syncwarp();
                 }
-                __syncwarp();
-            }
-            // while the MMA runs: this thread's X row, transposed into the B operand of eq. 8
+            };
+            if constexpr (!BF16) issue_eq1();                  // TF32: the tile is the operand as TMA delivered it
+            // this thread's part of its X row: BF16 copy for eq. 1, transposed into the B operand of eq. 8
             {
-                float xr[kIn];
+                float xr[4 * NCH];
 #pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    const float4 v = *reinterpret_cast<const float4*>(Xt_tile + swz(frow, c));
+                for (int c = 0; c < NCH; ++c) {
+                    const float4 v = *reinterpret_cast<const float4*>(Xtile + swz(frow, c0 + c));
                     xr[4 * c] = v.x; xr[4 * c + 1] = v.y; xr[4 * c + 2] = v.z; xr[4 * c + 3] = v.w;
                 }
+                if constexpr (BF16) {
 #pragma unroll
-                for (int i = 0; i < kIn; ++i)
-                    *reinterpret_cast<float*>(Xt + ka * (32 * 128) + swz(i, kk >> 2) + (kk & 3) * 4) = xr[i];
+                    for (int c = 0; c < NCH / 2; ++c)          // 16-byte chunk c0/2 + c holds inputs 8 (c0/2 + c) .. + 7
+                        *reinterpret_cast<uint4*>(Xb + swz(frow, c0 / 2 + c)) = pack_bf16x8(xr + 8 * c);
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    __syncthreads();                           // every row of the BF16 copy is written
+                    issue_eq1();
+                }
+#pragma unroll
+                for (int i = 0; i < 4 * NCH; ++i) {
+                    if constexpr (BF16) *reinterpret_cast<unsigned short*>(t8(Xt, 4 * c0 + i, 32)) = bf16_bits(xr[i]);
+                    else *reinterpret_cast<float*>(t8(Xt, 4 * c0 + i, 32)) = xr[i];
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp no longer reads the X tile
             mbar_wait(bar_mma, gt & 1u);
             tc_fence_after();
-            float mk[kIn];                                     // ReLU'(z_u) w2_u of this row (eq. 7 factor, old W2)
+            float mk[32];                                      // ReLU'(z_u) w2_u of this row (eq. 7 factor, old W2)
             {
                 uint32_t z[32];
                 tmem_ld32(taddr, z);
@@ -220,11 +285,11 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 float pr[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
                 for (int c = 0; c < 8; ++c) {
-                    const float4 w = *reinterpret_cast<const float4*>(W2s + 4 * c);
+                    const float4 w = *reinterpret_cast<const float4*>(W2s + uoff + 4 * c);
                     float4 h;
                     h.x = fmaxf(__uint_as_float(z[4 * c]), 0.f);      h.y = fmaxf(__uint_as_float(z[4 * c + 1]), 0.f);   // eq. 2
                     h.z = fmaxf(__uint_as_float(z[4 * c + 2]), 0.f);  h.w = fmaxf(__uint_as_float(z[4 * c + 3]), 0.f);
-                    *reinterpret_cast<float4*>(Hs + swz(frow, c)) = h;
+                    *reinterpret_cast<float4*>(Hs + hb * (BT * 128) + swz(frow, c)) = h;
                     mk[4 * c] = h.x > 0.f ? w.x : 0.f;     mk[4 * c + 1] = h.y > 0.f ? w.y : 0.f;
                     mk[4 * c + 2] = h.z > 0.f ? w.z : 0.f; mk[4 * c + 3] = h.w > 0.f ? w.w : 0.f;
                     pr[c & 3] = fmaf(h.x, w.x, fmaf(h.y, w.y, fmaf(h.z, w.z, fmaf(h.w, w.w, pr[c & 3]))));   // eq. 3
@@ -233,25 +298,27 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 #pragma unroll
                 for (uint32_t dd = 0; dd < C; ++dd) {          // one hop to every CTA of the cluster
                     const uint32_t d = (crank + dd) & (C - 1);
-                    st_async_f32(mapa(ypp_a + (buf * (C * BT) + crank * BT + frow) * 4, d), pv, mapa(yp_a + 8 * buf, d));
+                    st_async_f32(mapa(ypp_a + (buf * (NSL * BT) + (crank * NTH + hb) * BT + frow) * 4, d), pv, mapa(yp_a + 8 * buf, d));
                 }
             }
             // ---------------- eq. 5, eq. 7 ----------------
             mbar_wait(bar_yp + 8 * buf, ph);
             {
-                const float* ypt = ypp + buf * (C * BT);
-                float ypc[C];
+                const float* ypt = ypp + buf * (NSL * BT);
+                float ypc[NSL];
 #pragma unroll
-                for (int c = 0; c < C; ++c) ypc[c] = ypt[c * BT + frow];
+                for (int c = 0; c < NSL; ++c) ypc[c] = ypt[c * BT + frow];
 #pragma unroll
-                for (int o = 1; o < C; o <<= 1)
+                for (int o = 1; o < NSL; o <<= 1)              // fixed pairwise tree over the partial slots
 #pragma unroll
-                    for (int c = 0; c + o < C; c += 2 * o) ypc[c] += ypc[c + o];
+                    for (int c = 0; c + o < NSL; c += 2 * o) ypc[c] += ypc[c + o];
                 const float d = frow < vt ? scale * (ypc[0] - ycur) : 0.f;
-                Ds[frow] = d;
+                if (hb == 0) Ds[frow] = d;
 #pragma unroll
-                for (int u = 0; u < S; ++u)                    // dZ1^T[u][row]: A operand of eq. 8
-                    *reinterpret_cast<float*>(At + ka * (64 * 128) + swz(u, kk >> 2) + (kk & 3) * 4) = d * mk[u];
+                for (int u = 0; u < 32; ++u) {                 // dZ1^T[u][row]: A operand of eq. 8
+                    if constexpr (BF16) *reinterpret_cast<unsigned short*>(t8(At, uoff + u, 64)) = bf16_bits(d * mk[u]);
+                    else *reinterpret_cast<float*>(t8(At, uoff + u, 64)) = d * mk[u];
+                }
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // At, Xt (generic writes) -> MMA
             __syncthreads();
@@ -264,20 +331,24 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                         const uint64_t adesc = smem_desc_sw128(smem_u32(At) + a * (64 * 128));
                         const uint64_t bdesc = smem_desc_sw128(smem_u32(Xt) + a * (32 * 128));
 #pragma unroll
-                        for (int k = 0; k < 4; ++k)
-                            mma_tf32(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
+                        for (int k = 0; k < 4; ++k) {
+                            if constexpr (BF16) mma_f16(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
+                            else mma_tf32(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
+                        }
                     }
                     tc_commit(bar_mma2);
                 }
                 __syncwarp();
             }
-            // meanwhile eq. 6 on the CUDA cores: unit = lane, rows 32*warp .. 32*warp+31 of the tile
+            // meanwhile eq. 6 on the CUDA cores: one unit per lane, 32 rows of the tile per warp
             {
+                const int rbase = NTH == 1 ? warp * 32 : wq * 32;
+                const unsigned char* Hh = Hs + hb * (BT * 128);
                 float gp[4] = {0.f, 0.f, 0.f, 0.f};            // four independent chains hide the LDS latency
 #pragma unroll
                 for (int r = 0; r < 32; ++r) {
-                    const int row = warp * 32 + r;
-                    gp[r & 3] = fmaf(*reinterpret_cast<const float*>(Hs + swz(row, lane >> 2) + (lane & 3) * 4), Ds[row], gp[r & 3]);
+                    const int row = rbase + r;
+                    gp[r & 3] = fmaf(*reinterpret_cast<const float*>(Hh + swz(row, lane >> 2) + (lane & 3) * 4), Ds[row], gp[r & 3]);
                 }
                 g2 += (gp[0] + gp[1]) + (gp[2] + gp[3]);
             }
@@ -288,9 +359,9 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
         }
 
         // ---------------- end of batch: eq. 9 ----------------
-        part2[warp * S + lane] = g2;
+        part2[warp * 32 + lane] = g2;
         __syncthreads();
-        if (warp < 2) {                                        // owners of the eq. 8 accumulator rows
+        if (warp < S / 16) {                                   // owners of the eq. 8 accumulator rows
             uint32_t dw[32];
             tmem_ld32(tdw, dw);
             tmem_ld_wait();
@@ -300,11 +371,17 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 for (int i = 0; i < kIn; ++i) wrow[i] = fmaf(-p.lr, __uint_as_float(dw[i]), wrow[i]);   // W - lr*dW
                 store_wop();
             }
-        } else if (warp == 2) {                                // meanwhile eq. 9 for W2 (unit = lane)
-            float sum = part2[lane];
+        } else if (warp >= 4 && warp < 4 + S / 32) {           // meanwhile eq. 9 for W2 (one unit per lane)
+            const int hbw = warp - 4;                          // S = 32: warp 4, all 8 row blocks; S = 64: warps 4, 5
+            float sum = 0.f;
+            if constexpr (NTH == 1) {
 #pragma unroll
-            for (int w = 1; w < kWarps; ++w) sum += part2[w * S + lane];
-            W2s[lane] -= p.lr * sum;
+                for (int w = 0; w < kWarps; ++w) sum += part2[w * 32 + lane];
+            } else {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) sum += part2[(hbw * 4 + q) * 32 + lane];
+            }
+            W2s[hbw * 32 + lane] -= p.lr * sum;
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // Wop -> next step's MMA
         __syncthreads();
@@ -330,16 +407,62 @@ k_train_tf32(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
 }  // namespace
 
+// hidden 32..256: 32 units per CTA on hidden/32 CTAs; hidden 512 / 1024: 64 units per CTA on 8 / 16 CTAs
 bool train_tc_supported(int hidden, bool bf16) {
-    if (bf16) return false;
-    return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256;
+    (void)bf16;
+    return hidden == 32 || hidden == 64 || hidden == 128 || hidden == 256 || hidden == 512 || hidden == 1024;
 }
+
+namespace {
+
+template <int C, int S, bool BF16>
+cudaError_t launch_one(const float* X, int64_t n, const TcParams& p, cudaStream_t stream) {
+    using P = TcPlan<C, S, BF16>;
+    static_assert(P::BYTES <= 227 * 1024, "shared-memory plan exceeds the per-CTA limit");
+    if (n > 0x7fffffffLL - P::BT) return cudaErrorInvalidValue;          // TMA coordinates are int32
+    alignas(64) CUtensorMap tmap;
+    if (!make_x_tensormap(&tmap, X, n, P::BT)) return cudaErrorNotSupported;
+    auto kern = k_train_tc<C, S, BF16>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::BYTES);
+    if (e != cudaSuccess) return e;
+    if (C > 8) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(C);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = P::BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, tmap, p);
+}
+
+template <bool BF16>
+cudaError_t launch_width(const float* X, int64_t n, const TcParams& p, int hidden, cudaStream_t stream) {
+    switch (hidden) {
+        case 32: return launch_one<1, 32, BF16>(X, n, p, stream);
+        case 64: return launch_one<2, 32, BF16>(X, n, p, stream);
+        case 128: return launch_one<4, 32, BF16>(X, n, p, stream);
+        case 256: return launch_one<8, 32, BF16>(X, n, p, stream);
+        case 512: return launch_one<8, 64, BF16>(X, n, p, stream);
+        case 1024: return launch_one<16, 64, BF16>(X, n, p, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
 
 cudaError_t launch_train_tc(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
                             float* W1, float* W2, const int32_t* order, int hidden, bool bf16,
                             unsigned long long* stats, cudaStream_t stream, int64_t* launches) {
-    if (!train_tc_supported(hidden, bf16) || n > 0x7fffffffLL - kBT) return cudaErrorInvalidValue;
-    const int C = hidden / kS;
+    if (!train_tc_supported(hidden, bf16)) return cudaErrorInvalidValue;
     TcParams p;
     p.Y = Y; p.n = n; p.B = batch; p.lr = lr;
     const long long nb = (n + batch - 1) / batch;
@@ -350,39 +473,7 @@ cudaError_t launch_train_tc(const float* X, const float* Y, int64_t n, int batch
     p.scale_last = 2.0f / (float)p.m_last;
     p.W1 = W1; p.W2 = W2; p.order = order; p.H = hidden; p.stats = stats;
     if (p.total_steps == 0) return cudaSuccess;
-    alignas(64) CUtensorMap tmap;
-    if (!make_x_tensormap(&tmap, X, n, kBT)) return cudaErrorNotSupported;
-    const size_t smem = (size_t)kRing * kXBytes + kS * 128 + (kBT / 32) * 64 * 128 + (kBT / 32) * 32 * 128 + kBT * 128 +
-                        sizeof(float) * (2 * C * kBT + kWarps * kS + kS + kBT) + 8 * (2 * kRing + 4) + 16;
-    auto launch = [&](auto kern) -> cudaError_t {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        if (C > 8) {
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-            if (e != cudaSuccess) return e;
-        }
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(C);
-        cfg.blockDim = dim3(kThreads);
-        cfg.dynamicSmemBytes = smem;
-        cfg.stream = stream;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = C;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, kern, tmap, p);
-    };
-    cudaError_t err;
-    switch (C) {
-        case 1: err = launch(k_train_tf32<1>); break;
-        case 2: err = launch(k_train_tf32<2>); break;
-        case 4: err = launch(k_train_tf32<4>); break;
-        case 8: err = launch(k_train_tf32<8>); break;
-        default: return cudaErrorInvalidValue;
-    }
+    const cudaError_t err = bf16 ? launch_width<true>(X, n, p, hidden, stream) : launch_width<false>(X, n, p, hidden, stream);
     if (err == cudaSuccess) ++*launches;
     return err;
 }

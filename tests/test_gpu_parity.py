@@ -130,54 +130,60 @@ def test_train_rows_sample_level_shuffle(hidden, batch, n, epochs):
     assert torch.equal(dX, dev(X)) and torch.equal(dY, dev(Y))            # inputs untouched
 
 
-# Tensor-core training variant (TF32 forward): separately reported, stated
-# tolerance 5e-5 after one step, 2e-3 after one epoch, loss within 1 %.
-def test_train_tf32_variant_one_step_and_epoch(cfg1):
+# Tensor-core training variants (eqs. 1 and 8 on tcgen05): separately reported, stated
+# tolerances: TF32 5e-5 after one step, 2e-3 after one epoch; BF16 1e-4 / 5e-3; loss within 1 %.
+TC_VARIANTS = {"tf32": (B.VARIANT_TF32, 5e-5, 2e-3), "bf16": (B.VARIANT_BF16, 1e-4, 5e-3)}
+
+
+@pytest.mark.parametrize("mode", ["tf32", "bf16"])
+def test_train_tc_variant_one_step_and_epoch(cfg1, mode):
+    v, tol1, tole = TC_VARIANTS[mode]
     X, Y, W1, W2 = cfg1
-    g1, g2 = gpu_train(X[:256], Y[:256], W1, W2, 256, LR, 1, variant=B.VARIANT_TF32)
+    g1, g2 = gpu_train(X[:256], Y[:256], W1, W2, 256, LR, 1, variant=v)
     o1, o2 = O.train(X[:256], Y[:256], W1, W2, 256, LR, 1)
-    assert nerr(g1, o1) <= 5e-5 and nerr(g2, o2) <= 5e-5, (nerr(g1, o1), nerr(g2, o2))
+    assert nerr(g1, o1) <= tol1 and nerr(g2, o2) <= tol1, (nerr(g1, o1), nerr(g2, o2))
     c = datagen.CONFIGS["config2"]
     X, Y = datagen.make_dataset(c.n, c.sigma)
     order = datagen.make_order(c.n, c.batch, c.epochs, True)
-    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1], variant=B.VARIANT_TF32)
+    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1], variant=v)
     o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, 1, order=order[:1])
-    assert nerr(g1, o1) <= 2e-3 and nerr(g2, o2) <= 2e-3, (nerr(g1, o1), nerr(g2, o2))
-    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order, variant=B.VARIANT_TF32)
+    assert nerr(g1, o1) <= tole and nerr(g2, o2) <= tole, (nerr(g1, o1), nerr(g2, o2))
+    g1, g2 = gpu_train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order, variant=v)
     o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order)
     lg, lo = gpu_eval(X, Y, g1, g2), O.eval_loss(X, Y, o1, o2)
     assert abs(lg - lo) <= 1e-2 * lo, (lg, lo)
 
 
+@pytest.mark.parametrize("mode", ["tf32", "bf16"])
+@pytest.mark.parametrize("hidden", [256, 512])
 @pytest.mark.parametrize("batch,n", [(32, 2048), (1024, 8192), (100, 1001), (300, 1000), (5000, 3000), (1, 7)])
-def test_train_tf32_variant_batches_and_ragged(batch, n):
+def test_train_tc_variant_batches_and_ragged(batch, n, hidden, mode):
+    v, _, tole = TC_VARIANTS[mode]
     X, Y = datagen.make_dataset(n, 0.1)
-    W1, W2 = O.init_weights(2, 32, 256)
+    W1, W2 = O.init_weights(2, 32, hidden)
     order = datagen.make_order(n, batch, 2, True)
     o1, o2 = O.train(X, Y, W1, W2, batch, LR, 2, order=order)
-    g1, g2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=B.VARIANT_TF32)
-    assert nerr(g1, o1) <= 2e-3 and nerr(g2, o2) <= 2e-3, (batch, n, nerr(g1, o1), nerr(g2, o2))
-    h1, h2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=B.VARIANT_TF32)
+    g1, g2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=v)
+    assert nerr(g1, o1) <= tole and nerr(g2, o2) <= tole, (batch, n, nerr(g1, o1), nerr(g2, o2))
+    h1, h2 = gpu_train(X, Y, W1, W2, batch, LR, 2, order=order, variant=v)
     assert np.array_equal(g1, h1) and np.array_equal(g2, h2)              # deterministic
 
 
-@pytest.mark.parametrize("hidden", [32, 64, 128])
-def test_train_tf32_variant_hidden_sweep(hidden):
+@pytest.mark.parametrize("mode", ["tf32", "bf16"])
+@pytest.mark.parametrize("hidden", [32, 64, 128, 256, 512, 1024])
+def test_train_tc_variant_hidden_sweep(hidden, mode):
+    """Every width of the paper's sweep: the one-step gate and a 32-step run."""
+    v, tol1, tole = TC_VARIANTS[mode]
     n = 4096
     X, Y = datagen.make_dataset(n, 0.1)
     W1, W2 = O.init_weights(2, 32, hidden)
+    o1, o2 = O.train(X[:256], Y[:256], W1, W2, 256, LR, 1)
+    g1, g2 = gpu_train(X[:256], Y[:256], W1, W2, 256, LR, 1, variant=v)
+    assert nerr(g1, o1) <= tol1 and nerr(g2, o2) <= tol1, (hidden, nerr(g1, o1), nerr(g2, o2))
     order = datagen.make_order(n, 256, 2, True)
     o1, o2 = O.train(X, Y, W1, W2, 256, LR, 2, order=order)
-    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 2, order=order, variant=B.VARIANT_TF32)
-    assert nerr(g1, o1) <= 2e-3 and nerr(g2, o2) <= 2e-3, (hidden, nerr(g1, o1), nerr(g2, o2))
-
-
-def test_train_tf32_variant_unsupported_hidden():
-    X, Y = datagen.make_dataset(512, 0.1)
-    for hidden in (512, 1024):
-        W1, W2 = O.init_weights(2, 32, hidden)
-        with pytest.raises(B.MlpError):
-            gpu_train(X, Y, W1, W2, 256, LR, 1, variant=B.VARIANT_TF32)
+    g1, g2 = gpu_train(X, Y, W1, W2, 256, LR, 2, order=order, variant=v)
+    assert nerr(g1, o1) <= tole and nerr(g2, o2) <= tole, (hidden, nerr(g1, o1), nerr(g2, o2))
 
 
 # ------------------------------------------------------------------ config 2 (shuffled batch order)
