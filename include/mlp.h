@@ -53,14 +53,16 @@ enum {
     MLP_VARIANT_FUSED = 0,    /* training: persistent fused cluster kernel, exact fp32 (FFMA)   */
                               /* eval:     streaming fp32 kernel (FFMA)                          */
     MLP_VARIANT_UNFUSED = 1,  /* training: one kernel per equation, launched per step (baseline) */
-    MLP_VARIANT_TF32 = 2,     /* eval and training: eq. 1 on the tensor cores (tcgen05, TF32 operands, fp32
-                                 accumulate); separately reported, own tolerance; training: hidden <= 256 */
+    MLP_VARIANT_TF32 = 2,     /* eval: eq. 1, training: eqs. 1 and 8 on the tensor cores (tcgen05.mma kind::tf32: fp32
+                                 operands truncated to TF32, fp32 accumulate, fp32 master weights); separately
+                                 reported, own tolerance; every supported hidden width */
     MLP_VARIANT_PRIOR_NAIVE = 3, /* training: the paper's baseline, naive 16x16 matmul kernels; comparison only */
     MLP_VARIANT_PRIOR_TILED = 4, /* training: the paper's optimised strategy, tiled + transposed + fused ReLU; comparison only */
     MLP_VARIANT_BF16 = 5,     /* eval and training: as MLP_VARIANT_TF32 with BF16 operands (converted in the kernel, round to
                                  nearest even; tcgen05.mma kind::f16, fp32 accumulate); separately reported, own tolerance */
-    MLP_VARIANT_TF32X3 = 6    /* eval only: eq. 1 as three TF32 products (X = Xh + Xl, W = Wh + Wl; Xh Wh + Xh Wl + Xl Wh),
-                                 fp32-faithful to ~1e-6; separately reported */
+    MLP_VARIANT_TF32X3 = 6    /* eval only, hidden <= 256: eq. 1 as three TF32 products (X = Xh + Xl, W = Wh + Wl;
+                                 Xh Wh + Xl Wh + Xh Wl), fp32-faithful (loss within 1e-5 of the exact value);
+                                 separately reported */
 };
 
 /*
@@ -104,7 +106,7 @@ int mlp_train(const float* X, const float* Y, int64_t n, int batch, float lr, in
  *                validate the table on the host and return MLP_ERR_BAD_ARG before any work.
  *   variant:     MLP_VARIANT_FUSED, MLP_VARIANT_UNFUSED, MLP_VARIANT_PRIOR_NAIVE, MLP_VARIANT_PRIOR_TILED, or
  *                MLP_VARIANT_TF32 (stated tolerance vs the exact path: weights within 5e-5 after one step,
- *                2e-3 after one epoch, loss within 1 %).
+ *                2e-3 after one epoch, loss within 1 %), or MLP_VARIANT_BF16 (1e-4 / 5e-3 / 1 %).
  */
 int mlp_train_ex(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
                  float* W1, float* W2, const int32_t* batch_order, int variant, void* stream);
@@ -135,7 +137,10 @@ double mlp_eval_loss(const float* X, const float* Y, int64_t n,
  *   variant: MLP_VARIANT_FUSED = the exact-fp32 kernel of mlp_eval_loss (bound by the FP32 pipes);
  *            MLP_VARIANT_TF32  = eq. 1 on the tensor cores (tcgen05.mma kind::tf32: fp32 operands
  *            truncated to TF32, fp32 accumulate), the HBM-bound variant; stated tolerance: loss within
- *            1 % of the exact value (measured <= 1e-4 relative); n < 2^31 - 128, otherwise MLP_ERR_CUDA.  X must be 16-byte aligned.  Deterministic. */
+ *            1 % of the exact value (measured <= 1e-4 relative); n < 2^31 - 128, otherwise MLP_ERR_CUDA.
+ *            MLP_VARIANT_BF16  = the same with BF16 operands (rounded to nearest even in the kernel), loss within 1 %;
+ *            MLP_VARIANT_TF32X3 = three TF32 products, loss within 1e-5 of the exact value, hidden <= 256
+ *            (MLP_ERR_UNSUPPORTED otherwise).  X must be 16-byte aligned.  Deterministic. */
 int mlp_eval_loss_async(const float* X, const float* Y, int64_t n, const float* W1,
                         const float* W2, double* d_out, int variant, void* stream);
 

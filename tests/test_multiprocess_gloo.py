@@ -61,9 +61,9 @@ def test_sharded_eval_and_replica_timing_world2(n):
     procs = [ctx.Process(target=_worker, args=(r, 2, port, n, q)) for r in range(2)]
     for p in procs:
         p.start()
-    res = sorted(q.get(timeout=120) for _ in range(2))
+    res = sorted(q.get(timeout=600) for _ in range(2))
     for p in procs:
-        p.join(timeout=60)
+        p.join(timeout=120)
         assert p.exitcode == 0
     X, Y = datagen.make_dataset(n, 0.1)
     W1, W2 = O.init_weights(2, 32, 64)
