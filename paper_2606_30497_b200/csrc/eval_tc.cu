@@ -12,8 +12,9 @@
 //
 // Persistent grid, one CTA per SM, warp-specialised:
 //   warp 0      TMA producer: 128-row X tiles (16 KB) by cp.async.bulk.tensor with the 128-byte
-//               swizzle the MMA wants, into a kStages-deep ring;
-//   warps 11-14 (BF16 / TF32X3 only) converters: a thread owns one row of the landed tile;
+//               swizzle the MMA wants, into a kStages-deep ring; in the BF16 / TF32X3 modes this warp
+//               and warp 11 convert every landed tile (half a tile each, a lane owns two rows) before
+//               the MMA may read it (more converter warps would cap the epilogue's registers at 128);
 //   warp 1, 10  MMA issuers (even / odd tiles): per tile and column part four tcgen05.mma
 //               (M=128, N=hidden/NH, K=8) into the TMEM accumulator of that tile parity
 //               (2 x 256 columns = all of TMEM); tcgen05.commit releases the ring slot and
@@ -36,7 +37,7 @@ namespace {
 constexpr int kTile = 128;           // rows per MMA (M)
 constexpr int kStages = 6;           // X ring depth (6 x 16 KB)
 constexpr int kEvalThreads = 352;    // producer + MMA (even tiles) + 8 epilogue warps + MMA (odd tiles)
-constexpr int kConvThreads = 128;    // converter warps of the BF16 / TF32X3 modes (one thread per tile row)
+constexpr int kEvalThreadsConv = 384; // + the second converter warp of the BF16 / TF32X3 modes
 enum { kModeTf32 = 0, kModeBf16 = 1, kModeTf32x3 = 2 };
 constexpr uint32_t kTileBytes = kTile * kIn * 4;
 
@@ -46,7 +47,7 @@ constexpr uint32_t kTileBytes = kTile * kIn * 4;
 constexpr int eval_stages(int H, int mode) { return (H >= 1024 || mode == kModeTf32x3) ? 4 : kStages; }
 
 template <int H, int MODE>
-__global__ void __launch_bounds__(kEvalThreads + (MODE == kModeTf32 ? 0 : kConvThreads), 1)
+__global__ void __launch_bounds__(MODE == kModeTf32 ? kEvalThreads : kEvalThreadsConv, 1)
 k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y, long long n,
             const float* __restrict__ W1, const float* __restrict__ W2,
             double* __restrict__ partials, unsigned int* __restrict__ ticket,
@@ -77,7 +78,7 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
                    bar_conv = smem_u32(bars + 2 * NST + 16);               // [NST] tile converted (BF16 / TF32X3)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NW = (kEvalThreads + (MODE == kModeTf32 ? 0 : kConvThreads)) / 32;
+    constexpr int NW = (MODE == kModeTf32 ? kEvalThreads : kEvalThreadsConv) / 32;
     __shared__ int last_flag_s;
     int* last_flag = &last_flag_s;
 
@@ -92,7 +93,7 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
     if (tid == 0) {
         for (int s = 0; s < NST; ++s) {
             mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, NS > 1 ? 2 : 1);
-            mbar_init(bar_conv + 8 * s, kConvThreads / 32);
+            mbar_init(bar_conv + 8 * s, 2);
         }
         for (int b = 0; b < 8; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
         fence_mbar_init();
@@ -176,19 +177,63 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
     // (w & 1), MMA issuer (w & 1) and epilogue set (w & 1).  nt * NS < 2^31 by the host check.
     const uint32_t nitems = nt * NS;
 
+    // BF16 / TF32X3: warp 0 (rows 0-63) and warp 11 (rows 64-127) convert every landed tile, a lane owns two rows of its half
+    auto convert_half = [&](uint32_t i, int half) {
+        const uint32_t st = i % NST;
+        mbar_wait(bar_full + 8 * st, (i / NST) & 1u);
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) {
+            const int r = half * 64 + rr * 32 + lane;
+            unsigned char* row = Xring + st * kTileBytes + r * 128;
+            float4 v[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) v[c] = *reinterpret_cast<const float4*>(row + ((c ^ (r & 7)) << 4));
+            if constexpr (MODE == kModeBf16) {                          // in place: 32 bf16 in the first 64 logical bytes
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    *reinterpret_cast<uint4*>(row + ((c ^ (r & 7)) << 4)) =
+                        make_uint4(bf16x2(v[2 * c].x, v[2 * c].y), bf16x2(v[2 * c].z, v[2 * c].w),
+                                   bf16x2(v[2 * c + 1].x, v[2 * c + 1].y), bf16x2(v[2 * c + 1].z, v[2 * c + 1].w));
+            } else {                                                    // value exact in TF32 in place, residual beside it
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    *reinterpret_cast<float4*>(row + ((c ^ (r & 7)) << 4)) =
+                        make_float4(tf32_trunc(v[c].x), tf32_trunc(v[c].y), tf32_trunc(v[c].z), tf32_trunc(v[c].w));
+                    *reinterpret_cast<float4*>(row + NST * kTileBytes + ((c ^ (r & 7)) << 4)) =
+                        make_float4(tf32_residual(v[c].x), tf32_residual(v[c].y), tf32_residual(v[c].z), tf32_residual(v[c].w));
+                }
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes -> MMA (async proxy)
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_conv + 8 * st);
+    };
     if (warp == 0) {
         // ===== TMA producer (whole warp runs the loop, one elected lane issues) =====
-        uint32_t st = 0, eph = 0;                       // ring stage, parity of the "empty" phase to wait for
-        for (uint32_t i = NST; i < nt; ++i) {           // tiles 0..NST-1 were issued before the set-up
-            mbar_wait(bar_empty + 8 * st, eph);
+        auto refill = [&](uint32_t i) {                 // tile i goes into the slot tile i - NST has left
+            const uint32_t st = i % NST;
+            mbar_wait(bar_empty + 8 * st, ((i / NST) - 1u) & 1u);
             if (elect_one()) {
                 const long long row0 = (blockIdx.x + (long long)i * gridDim.x) * kTile;
                 mbar_arrive_expect_tx(bar_full + 8 * st, kTileBytes);   // OOB rows are zero-filled, still counted
                 tma_load_2d(smem_u32(Xring) + st * kTileBytes, &tmapX, 0, (int)row0, bar_full + 8 * st);
             }
             __syncwarp();
-            if (++st == NST) { st = 0; eph ^= 1u; }
+        };
+        if constexpr (MODE == kModeTf32) {
+            for (uint32_t i = NST; i < nt; ++i) refill(i);   // tiles 0..NST-1 were issued before the set-up
+        } else {
+            // ... and converter: tile i is converted as soon as it has landed; the slot of tile i - 1 is refilled
+            // afterwards (its MMA has had a whole conversion to finish), so the two duties never wait on each other
+            for (uint32_t i = 0; i < nt; ++i) {
+                const uint32_t st = i % NST;
+                convert_half(i, 0);
+                if (i >= 1 && i - 1 + NST < nt) refill(i - 1 + NST);
+            }
         }
+    } else if (warp == 11) {
+        if constexpr (MODE != kModeTf32)
+            for (uint32_t i = 0; i < nt; ++i) convert_half(i, 1);
     } else if (warp == 1 || warp == 10) {
         // ===== MMA issuers: warp 1 feeds accumulator 0 (even items), warp 10 accumulator 1 (odd items), so
         // that neither epilogue set ever waits behind the other set's TMEM hand-back (whole warp runs
@@ -233,37 +278,6 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
                     tc_commit(bar_tfull + 8 * (NH * b + hf));           // accumulator part ready
                 }
                 __syncwarp();
-            }
-        }
-    } else if (warp >= kEvalThreads / 32) {
-        // ===== converters (BF16 / TF32X3): a thread owns one row of every landed tile =====
-        if constexpr (MODE != kModeTf32) {
-            const int r = tid - kEvalThreads;                                   // tile row 0..127
-            for (uint32_t i = 0; i < nt; ++i) {
-                const uint32_t st = i % NST;
-                mbar_wait(bar_full + 8 * st, (i / NST) & 1u);
-                unsigned char* row = Xring + st * kTileBytes + r * 128;
-                float4 v[8];
-#pragma unroll
-                for (int c = 0; c < 8; ++c) v[c] = *reinterpret_cast<const float4*>(row + ((c ^ (r & 7)) << 4));
-                if constexpr (MODE == kModeBf16) {                              // in place: 32 bf16 in the first 64 logical bytes
-#pragma unroll
-                    for (int c = 0; c < 4; ++c)
-                        *reinterpret_cast<uint4*>(row + ((c ^ (r & 7)) << 4)) =
-                            make_uint4(bf16x2(v[2 * c].x, v[2 * c].y), bf16x2(v[2 * c].z, v[2 * c].w),
-                                       bf16x2(v[2 * c + 1].x, v[2 * c + 1].y), bf16x2(v[2 * c + 1].z, v[2 * c + 1].w));
-                } else {                                                        // value exact in TF32 in place, residual beside it
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) {
-                        *reinterpret_cast<float4*>(row + ((c ^ (r & 7)) << 4)) =
-                            make_float4(tf32_trunc(v[c].x), tf32_trunc(v[c].y), tf32_trunc(v[c].z), tf32_trunc(v[c].w));
-                        *reinterpret_cast<float4*>(row + NST * kTileBytes + ((c ^ (r & 7)) << 4)) =
-                            make_float4(tf32_residual(v[c].x), tf32_residual(v[c].y), tf32_residual(v[c].z), tf32_residual(v[c].w));
-                    }
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes -> MMA (async proxy)
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_conv + 8 * st);
             }
         }
     } else {
@@ -407,7 +421,7 @@ cudaError_t launch_hm(const CUtensorMap& tmap, const float* Y, long long n, cons
                         32 * 4 + 4 + 4 + 64;
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
-    kern<<<grid, kEvalThreads + (MODE == kModeTf32 ? 0 : kConvThreads), smem, stream>>>(tmap, Y, n, W1, W2, partials, ticket, d_out);
+    kern<<<grid, MODE == kModeTf32 ? kEvalThreads : kEvalThreadsConv, smem, stream>>>(tmap, Y, n, W1, W2, partials, ticket, d_out);
     return cudaGetLastError();
 }
 
