@@ -223,3 +223,34 @@ def test_eval_loss_host_chunked_pipeline(variant):
     assert a == B.mlp_eval_loss_host(X, Y, n, W1, W2, v)                 # deterministic
     lo = O.eval_loss(X, Y, W1, W2)
     assert abs(a - lo) <= (2e-6 if variant == "FUSED" else 5e-3) * lo
+
+
+@pytest.mark.parametrize("variant", ["FUSED", "TF32", "BF16"])
+def test_cluster_sizes_agree_under_load(variant):
+    """Stress test for the cross-CTA Ypred exchange (st.async + remote mbarrier transaction bytes, waited for with
+    a CTA-scope acquire): the whole of BASELINE.json config 2 (2,560 SGD steps) at every
+    cluster size, while a second stream keeps the rest of the chip busy with full-grid eval passes.  Every run
+    must match the oracle; a lost or early-read partial would show up as a wrong gradient."""
+    c = datagen.CONFIGS["config2"]
+    X, Y = datagen.make_dataset(c.n, c.sigma)
+    order = datagen.make_order(c.n, c.batch, c.epochs, True)
+    W1, W2 = O.init_weights(2, 32, c.hidden)
+    o1, o2 = O.train(X, Y, W1, W2, c.batch, LR, c.epochs, order=order)
+    B.mlp_init(2, 32, c.hidden, 1)
+    dX, dY, dO = dev(X), dev(Y), dev(order.reshape(-1))
+    v = getattr(B, "VARIANT_" + variant)
+    tol = {"FUSED": 1e-5, "TF32": 2e-3, "BF16": 5e-3}[variant]
+    side = torch.cuda.Stream()
+    e1, e2 = dev(W1), dev(W2)
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    for cl in ((2, 4, 8, 16) if variant == "FUSED" else (0,)):
+        B.mlp_set_cluster(cl)
+        d1, d2 = dev(W1), dev(W2)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            for _ in range(40):                                   # ~12 ms of full-grid work beside the training launch
+                B.mlp_eval_loss_async(dX, dY, c.n, e1, e2, sink, B.VARIANT_FUSED)
+        B.mlp_train_ex(dX, dY, c.n, c.batch, LR, c.epochs, d1, d2, dO, v)
+        torch.cuda.synchronize()
+        assert nerr(d1.cpu().numpy(), o1) <= tol and nerr(d2.cpu().numpy(), o2) <= tol, (variant, cl)
+    B.mlp_set_cluster(0)

@@ -389,6 +389,24 @@ def test_init_weights_distribution_and_determinism():
     u = (z >> 40) / 16777216.0
     assert W1[0, 0] == np.float32((2 * u - 1) * b1)
 
+    # the same by hand for other flat indices e (W1 row-major, then W2): an interior W1 element, the last W1
+    # element, the first W2 element (e = 32*256: the branch that switches offset and bound) and the last one
+    def by_hand(seed, e, bound):
+        z = (seed + 0x9E3779B97F4A7C15 * (e + 1)) & (2 ** 64 - 1)
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & (2 ** 64 - 1)
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & (2 ** 64 - 1)
+        z ^= z >> 31
+        return np.float32((2 * ((z >> 40) / 16777216.0) - 1) * bound)
+    assert W1[3, 17] == by_hand(2, 3 * 256 + 17, b1)
+    assert W1[31, 255] == by_hand(2, 32 * 256 - 1, b1)
+    assert W2[0] == by_hand(2, 32 * 256, b2)
+    assert W2[255] == by_hand(2, 32 * 256 + 255, b2)
+    for hidden in (32, 1024):                                   # the bound of W2 follows the hidden width
+        A1, A2 = O.init_weights(7, 32, hidden)
+        assert A2[0] == by_hand(7, 32 * hidden, 1 / math.sqrt(hidden))
+        assert A2[hidden - 1] == by_hand(7, 32 * hidden + hidden - 1, 1 / math.sqrt(hidden))
+        assert A1[31, hidden - 1] == by_hand(7, 32 * hidden - 1, b1)
+
 
 def test_state_fp64_switch_is_report_only():
     X, Y = datagen.make_dataset(4096, 0.1)
