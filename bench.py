@@ -422,8 +422,13 @@ def extras(line, B, datagen, roofline, torch, peaks, cfg, X_all, Y_all, dX_all, 
         for vname, v in (("tf32", B.VARIANT_TF32), ("bf16", B.VARIANT_BF16)):
             try:
                 tus, tsps, tfl = train_member(c, v)
+                tfloor = roofline.tc_train_floor_us(c.batch, c.hidden, mhz, vname == "bf16")
                 row["train_" + vname] = {"us_per_sgd_step": tus, "samples_per_s": tsps, "final_loss": tfl,
-                                         "final_loss_rel_diff_vs_fp32_path": abs(tfl - fl) / fl}
+                                         "final_loss_rel_diff_vs_fp32_path": abs(tfl - fl) / fl,
+                                         "cluster": roofline.tc_train_cluster(c.hidden),
+                                         "floor_us_per_sgd_step": tfloor, "frac_of_tc_floor": tfloor / tus,
+                                         "floor": "tensor time of eqs. 1, 8 at the nominal dense rate of the cluster's SMs "
+                                                  "+ other FLOP at the FP32-FMA rate + one DSMEM hop per tile (roofline.py)"}
             except B.MlpError:
                 row["train_" + vname] = None
         per[c.name] = row
