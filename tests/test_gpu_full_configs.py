@@ -18,6 +18,7 @@ from paper_2606_30497_b200 import binding as B          # noqa: E402
 from paper_2606_30497_b200 import datagen               # noqa: E402
 
 LR = np.float32(0.002)
+REPORT = {}          # measured errors per config member, written to gpurun_out/r02_parity_full_configs.json at exit
 
 
 def nerr(g, o):
@@ -56,6 +57,9 @@ def check_config(c, oracle_epochs):
     g1 = Gpu(X[lo:hi], Y[lo:hi], c.hidden).train(W1, W2, c.batch, 1, np.zeros((1, 1), np.int32))
     o1 = O.train(X[lo:hi], Y[lo:hi], W1, W2, c.batch, LR, 1)
     assert nerr(g1[0], o1[0]) <= 1e-5 and nerr(g1[1], o1[1]) <= 1e-5, (c.name, "1 step", nerr(g1[0], o1[0]))
+    rec = REPORT.setdefault(c.name, {"hidden": c.hidden, "batch": c.batch, "n": c.n, "epochs": c.epochs,
+                                     "oracle_epochs_compared": oracle_epochs})
+    rec["one_step_err_W1_W2"] = [nerr(g1[0], o1[0]), nerr(g1[1], o1[1])]
     # epoch by epoch, as far as the oracle is run
     gw, ow = (W1, W2), (W1, W2)
     losses = [g.loss(W1, W2)]
@@ -68,11 +72,25 @@ def check_config(c, oracle_epochs):
             assert e1 <= 1e-3 and e2 <= 1e-3, (c.name, "epoch", e + 1, e1, e2)
             lo_ = O.eval_loss(X, Y, ow[0], ow[1])
             assert abs(losses[-1] - lo_) <= 1e-2 * lo_, (c.name, "loss after epoch", e + 1, losses[-1], lo_)
+            if e == 0:
+                rec["one_epoch_err_W1_W2"] = [e1, e2]
+            rec["last_compared_epoch"] = {"epoch": e + 1, "err_W1_W2": [e1, e2], "loss_gpu": losses[-1], "loss_oracle": lo_,
+                                          "loss_rel_err": abs(losses[-1] - lo_) / lo_}
     assert all(b < a for a, b in zip(losses, losses[1:])), (c.name, losses)
     # the whole config in ONE launch (what bench.py times) equals the epoch-by-epoch runs bitwise
     w_all = g.train(W1, W2, c.batch, c.epochs, order)
     assert np.array_equal(w_all[0], gw[0]) and np.array_equal(w_all[1], gw[1]), c.name
     assert nb * c.epochs == order.size
+    rec["final_loss_gpu"] = losses[-1]
+    _dump_report()
+
+
+def _dump_report():
+    import json
+    import os
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(out):
+        json.dump(REPORT, open(os.path.join(out, "r02_parity_full_configs.json"), "w"), indent=1)
 
 
 def test_config3_full():
