@@ -45,7 +45,7 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback", "bf16_tflops": 1600.0}
 
 
-def workload_config(cfg, cluster=None, world=1):
+def workload_config(cfg):
     """The `config` object both arms print (same keys, same values: the same job)."""
     c = {"workload": WORKLOAD, "n": cfg.n, "hidden": cfg.hidden, "batch": cfg.batch, "epochs": cfg.epochs,
          "evals_per_step": cfg.epochs, "sgd_steps_per_step": cfg.epochs * ((cfg.n + cfg.batch - 1) // cfg.batch),
@@ -53,8 +53,7 @@ def workload_config(cfg, cluster=None, world=1):
                             "(per-epoch batch-order permutation, seed 3), an eval-loss pass over the dataset "
                             "after each epoch",
          "l2": "dataset (138 MB) larger than L2 (126 MB); L2 also flushed between timed steps (256 MiB memset, untimed)"}
-    if cluster is not None:
-        c["parallelism"] = "replicas only" if world > 1 else "1 GPU, cluster of %d SMs" % cluster
+    c["parallelism"] = "replicas only (one independent job per GPU; the SGD step does not shard)"
     return c
 
 
@@ -313,7 +312,7 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": workload_config(cfg, cluster, world),
+        "config": workload_config(cfg), "cluster_sms": cluster,
         "us_per_sgd_step": us_per_sgd, "epoch_losses": losses, "final_loss": losses[-1],
         "roofline": roof, "gpu_launches": int(launches), "clocks": sampler.summary(),
         "context": "paper (Tesla T4, optimised kernels): 1,482 us/step, 172.7 k samples/s (PAPER.md:330, derived)",
