@@ -6,28 +6,31 @@
 // whose fp32 master copy stays in shared memory for the whole run.
 //
 // Mapping inside a CTA (8 warps):
-//   * a lane owns FOUR hidden units (u_j = lu + j*LPS, lu = lane % LPS, LPS = S/4); a warp
-//     instruction covers SPW = 32/LPS rows (one per lane sub-group s = lane / LPS).  The X tile is
-//     stored as SPW blocks of BT/SPW rows, block s shifted by 16*s bytes, so the SPW rows read by
-//     one LDS.128 fall into distinct bank groups (no conflict, no swizzle);
-//   * forward (eqs. 1-3): the lane's four W1 columns (4 x 32 floats) live in registers for the
-//     forward pass only; one 128-bit shared-memory load of X feeds 8 FFMA2 (fma.rn.f32x2).  The
-//     first row group is processed chunk-major so the register reload of W1 (4 shared-memory
-//     cycles per LDS.128: ~1,000 cycles per CTA) overlaps its FMAs.  H = ReLU(Z1) of the warp's
-//     rows stays in registers between forward and backward;
+//   * a lane owns FOUR hidden units (u_j = lu + j*LPS, LPS = S/4 lanes per row); a warp instruction
+//     covers SPW = 32/LPS rows (sub-groups s).  Lane id = bit 0 of s, then lu, then the other bits of
+//     s: with this order both broadcast load patterns (X rows, W1 reload) cost 2 shared-memory
+//     wavefronts per LDS.128.  The X tile is stored as SPW blocks of BT/SPW rows, block s shifted by
+//     16*s bytes, so the SPW rows read by one LDS.128 fall into distinct bank groups;
+//   * forward (eqs. 1-3), K-split over lane pairs: lane lu and its partner lu ^ LPS/2 share their
+//     eight units and each takes one half of the 32 inputs: 8 columns x 16 inputs of W1 live in 128
+//     registers for the forward pass only, half an X row is read per lane (4 LDS.128 feed 64 FFMA2,
+//     fma.rn.f32x2) and the halves of Z1 meet by one shuffle per unit.  The first rows are processed
+//     chunk-major so the register reload of W1 overlaps their FMAs.  H = ReLU(Z1) of the warp's rows
+//     stays in registers between forward and backward;
 //   * per-row partial Ypred: transposing shuffle tree over the LPS lanes, then pushed to every CTA
 //     of the cluster with st.async (DSMEM store that completes transaction bytes on the
 //     destination's mbarrier: one hop, no flag), one fixed peer per lane, straight-line code (the
 //     cluster size is a template parameter).  The tile is processed as NSPLIT row groups so that
 //     the exchange of one group is in flight while the other group computes;
-//   * backward (eqs. 5-8), K-split: every CTA sums the C partials (fixed tree) -> dZ2; the lane of
-//     sub-group s accumulates dW1 only for inputs [IPS*s, IPS*(s+1)) of its four units (32
-//     registers at SPW = 4) but over the rows of ALL sub-groups, whose dZ1 arrives by shuffle: no
-//     reduction across sub-groups.  Per-warp partials go to shared memory; at the end of the batch
-//     the 8 warps' partials are summed by a fixed pairwise tree (deterministic) and eq. 9 is
-//     applied to the shared-memory master copy.
+//   * backward (eqs. 5-8), K-split over the sub-groups: every CTA sums the C partials (fixed tree)
+//     -> dZ2; the lane of sub-group s accumulates dW1 only for inputs [IPS*s, IPS*(s+1)) of its four
+//     units (32 registers at SPW = 4) but over the rows of ALL sub-groups, whose dZ1 arrives by
+//     shuffle: no reduction across sub-groups.  Per-warp partials go to shared memory; at the end of
+//     the batch the 8 warps' partials are summed by a fixed pairwise tree (deterministic) and eq. 9
+//     is applied to the shared-memory master copy.
 // X tiles arrive by cp.async.bulk (TMA engine) into a 3-stage ring, one tile ahead; Y one tile
-// ahead into a holder lane's register.  Measured: DESIGN.md 5.1, profiles/r01_ncu_v3.md.
+// ahead into a holder lane's register.  Measured: DESIGN.md 5.1, profiles/r02_ncu.md; the cost model
+// behind the mapping (loads and shuffles add to the FMA time): profiles/r02_microbench.md.
 #include "common.cuh"
 #include "internal.h"
 
@@ -228,9 +231,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                     __syncwarp();
                 }
             };
-#ifndef MLP_PRODUCER_LATE
             producer_duties();
-#endif
             float ynext = 0.f;
             if (yholder && yrow < nrows) ynext = __ldg(p.Y + nr0 + yrow);
 
@@ -323,10 +324,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                     }
                 }
             }
-
-#ifdef MLP_PRODUCER_LATE
-            producer_duties();
-#endif
 
             // ---------------- backward: eqs. 5-8 ----------------
             // K-split: the lane of sub-group s accumulates dW1 only for the IPS inputs
