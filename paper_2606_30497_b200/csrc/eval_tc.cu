@@ -436,7 +436,7 @@ cudaError_t launch_h(int mode, const CUtensorMap& tmap, const float* Y, long lon
 
 }  // namespace
 
-bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows) {
+bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows, bool atom32) {
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)kIn, (cuuint64_t)n};
@@ -444,7 +444,8 @@ bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows) {
     const cuuint32_t box[2] = {(cuuint32_t)kIn, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     return enc(static_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(X),
-               dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               atom32 ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : CU_TENSOR_MAP_SWIZZLE_128B,
                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

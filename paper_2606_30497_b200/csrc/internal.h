@@ -48,8 +48,9 @@ cudaError_t launch_eval_fp32(const float* X, const float* Y, int64_t n, const fl
                              double* d_out, cudaStream_t stream, int64_t* launches);
 
 // X viewed as a 2-D tensor [n][32] fp32 with 128-byte swizzle, box = box_rows rows (<= 256); *out_map is a
-// CUtensorMap (128 bytes, 64-byte aligned).  False if the driver entry point is unavailable.
-bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows);
+// CUtensorMap (128 bytes, 64-byte aligned).  False if the driver entry point is unavailable.  atom32: swizzle 32-byte
+// chunks (CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, the layout a TF32 operand needs to be readable MN-major) instead of 16-byte ones.
+bool make_x_tensormap(void* out_map, const float* X, int64_t n, int box_rows, bool atom32 = false);
 
 // train_tc.cu -- fused cluster training kernel with eqs. 1 and 8 on the tensor cores (row a-T, separately
 // reported): TF32 operands (fp32 bits truncated by the tensor core) or BF16 operands (converted in the kernel,

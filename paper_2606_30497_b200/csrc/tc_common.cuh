@@ -60,6 +60,20 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
 
+// The same tile geometry with the "128-byte swizzle, 32-byte atom" (CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B; UMMA layout type 1):
+// the 32-byte chunk index is XORed with (row & 3), the pattern repeats every 4 rows (512 bytes).  It is the layout in which
+// a TF32 operand can be read in EITHER orientation (measured with a probe kernel, profiles/r02_microbench.md section 4):
+//   K-major  (rows = M or N index, the 128 bytes of a row = 32 K elements): groups of 4 rows, SBO = 512 bytes; +32 bytes per K = 8;
+//   MN-major (rows = K index, the 128 bytes of a row = 32 M or N elements): groups of 4 K rows, SBO = 512 bytes, LBO = distance
+//            between 32-element column blocks of M / N; +1,024 bytes (8 rows) per K = 8; instruction-descriptor bit 15 (A) / 16 (B).
+// (The 16-byte-atom swizzle of smem_desc_sw128 gives all-zero results for MN-major TF32 operands; LBO must be 32-byte aligned.)
+__device__ __forceinline__ uint64_t smem_desc_sw128_a32(uint32_t saddr, uint32_t lbo_bytes) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | (32ull << 32) | (1ull << 46) | (1ull << 61);
+}
+// byte offset of the 16-byte half h of the 32-byte chunk g of row r in such a tile
+__device__ __forceinline__ int swz32(int r, int g, int h) { return r * 128 + ((g ^ (r & 3)) << 5) + (h << 4); }
+constexpr uint32_t kIdescAMajorMN = 1u << 15, kIdescBMajorMN = 1u << 16;
+
 // byte offset of the 16-byte chunk c of row r in a [rows][128 B] tile with the 128-byte swizzle
 __device__ __forceinline__ int swz(int r, int c) { return r * 128 + ((c ^ (r & 7)) << 4); }
 // two fp32 -> packed bf16x2 (round to nearest even); `lo` lands in the low half

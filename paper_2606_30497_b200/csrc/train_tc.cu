@@ -23,7 +23,11 @@
 //   (eq. 7) into the K-major A operand of eq. 8; warp 0 issues eq. 8 while all warps do eq. 6 (dW2) on
 //   the CUDA cores.  At the end of the batch the threads that own the TMEM rows of dW1^T (one per hidden
 //   unit) apply eq. 9 to the fp32 master row they keep in registers and rewrite their row of the eq. 1
-//   operand.  All operands are K-major with the 128-byte swizzle (the conventions of eval_tc.cu).
+//   operand.  BF16 mode: all operands K-major with the 128-byte swizzle (the conventions of eval_tc.cu), the two
+//   operands of eq. 8 transposed by the threads with 2-byte stores.  TF32 mode: the X tile arrives with the
+//   32-byte-atom flavour of the 128-byte swizzle, in which a TF32 operand can be read K-major (eq. 1) AND MN-major
+//   (tc_common.cuh): eq. 8 takes the tile itself as its B operand and dZ1 as the threads produce it (a row = 32
+//   units = 128 bytes) as its A operand: no transposing stores, the threads never read X.
 #include <cuda.h>
 
 #include "tc_common.cuh"
@@ -63,9 +67,9 @@ struct TcPlan {
     static constexpr uint32_t oX = 0;                                   // [kRing][BT][128 B]  A of eq. 1 (TF32)
     static constexpr uint32_t oXb = oX + kRing * XBYTES;                // [BT][128 B]         A of eq. 1 (BF16 copy)
     static constexpr uint32_t oW = oXb + (BF16 ? XBYTES : 0);           // [S][128 B]          B of eq. 1
-    static constexpr uint32_t oAt = oW + S * 128;                       // [NA][64][128 B]     A of eq. 8 (dZ1^T)
-    static constexpr uint32_t oXt = oAt + NA * 64 * 128;                // [NA][32][128 B]     B of eq. 8 (X^T)
-    static constexpr uint32_t oH = oXt + NA * 32 * 128;                 // [NTH][BT][128 B]    H = ReLU(Z1)
+    static constexpr uint32_t oAt = oW + S * 128;                       // A of eq. 8 (dZ1^T): BF16 [NA][64][128 B] K-major; TF32 [2][BT][128 B] MN-major
+    static constexpr uint32_t oXt = oAt + (BF16 ? NA * 64 * 128 : BT * 256);                     // B of eq. 8 (X^T): BF16 [NA][32][128 B]; TF32: the X tile itself, MN-major
+    static constexpr uint32_t oH = oXt + (BF16 ? NA * 32 * 128 : 0);    // [NTH][BT][128 B]    H = ReLU(Z1)
     static constexpr uint32_t oYp = oH + NTH * BT * 128;                // [2][NSL][BT] floats
     static constexpr uint32_t oP2 = oYp + 2 * NSL * BT * 4;             // [kWarps][32] dW2 partials
     static constexpr uint32_t oW2 = oP2 + kWarps * 32 * 4;              // [S]
@@ -136,10 +140,10 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
     // ---- one-time setup ---------------------------------------------------------------------------
     if (wowner) store_wop();
-    for (int f = tid; f < NA * 64 * 32; f += kThreads) reinterpret_cast<float*>(At)[f] = 0.f;   // padding rows stay 0
+    for (int f = tid; f < (int)(P::oXt - P::oAt) / 4; f += kThreads) reinterpret_cast<float*>(At)[f] = 0.f;   // padding rows / plane stay 0
     if (tid < S) W2s[tid] = p.W2[crank * S + tid];
     if (tid == 0) {
-        for (int b = 0; b < kRing; ++b) { mbar_init(bar_full + 8 * b, 1); mbar_init(bar_empty + 8 * b, kWarps); }
+        for (int b = 0; b < kRing; ++b) { mbar_init(bar_full + 8 * b, 1); mbar_init(bar_empty + 8 * b, BF16 ? kWarps : 1); }
         mbar_init(bar_yp, 1); mbar_init(bar_yp + 8, 1); mbar_init(bar_mma, 1); mbar_init(bar_mma2, 1);
         fence_mbar_init();
     }
@@ -237,7 +241,8 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                         const uint64_t bdesc = smem_desc_sw128(smem_u32(Wop));
 #pragma unroll
                         for (int a = 0; a < (NTH == 1 ? 2 : 1); ++a) {     // row blocks of 128 (S = 32: two of them)
-                            const uint64_t adesc = smem_desc_sw128((BF16 ? smem_u32(Xb) : smem_u32(Xs) + xst * kXBytes) + a * 128 * 128);
+                            const uint64_t adesc = BF16 ? smem_desc_sw128(smem_u32(Xb) + a * 128 * 128)
+                                                        : smem_desc_sw128_a32(smem_u32(Xs) + xst * kXBytes + a * 128 * 128, 1024);
 #pragma unroll
                             for (int k = 0; k < KS1; ++k) {
                                 if constexpr (BF16) mma_f16(tmem_base + a * 32, adesc + 2 * k, bdesc + 2 * k, idesc1, k > 0);
@@ -250,30 +255,26 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 }
             };
             if constexpr (!BF16) issue_eq1();                  // TF32: the tile is the operand as TMA delivered it
-            // this thread's part of its X row: BF16 copy for eq. 1, transposed into the B operand of eq. 8
-            {
+            // BF16: this thread's part of its X row: rounded copy for eq. 1, transposed into the B operand of eq. 8
+            // (TF32: the tile is read by the tensor core only, in both orientations; eq. 8's commit releases the slot)
+            if constexpr (BF16) {
                 float xr[4 * NCH];
 #pragma unroll
                 for (int c = 0; c < NCH; ++c) {
                     const float4 v = *reinterpret_cast<const float4*>(Xtile + swz(frow, c0 + c));
                     xr[4 * c] = v.x; xr[4 * c + 1] = v.y; xr[4 * c + 2] = v.z; xr[4 * c + 3] = v.w;
                 }
-                if constexpr (BF16) {
 #pragma unroll
-                    for (int c = 0; c < NCH / 2; ++c)          // 16-byte chunk c0/2 + c holds inputs 8 (c0/2 + c) .. + 7
-                        *reinterpret_cast<uint4*>(Xb + swz(frow, c0 / 2 + c)) = pack_bf16x8(xr + 8 * c);
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    __syncthreads();                           // every row of the BF16 copy is written
-                    issue_eq1();
-                }
+                for (int c = 0; c < NCH / 2; ++c)          // 16-byte chunk c0/2 + c holds inputs 8 (c0/2 + c) .. + 7
+                    *reinterpret_cast<uint4*>(Xb + swz(frow, c0 / 2 + c)) = pack_bf16x8(xr + 8 * c);
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncthreads();                           // every row of the BF16 copy is written
+                issue_eq1();
 #pragma unroll
-                for (int i = 0; i < 4 * NCH; ++i) {
-                    if constexpr (BF16) *reinterpret_cast<unsigned short*>(t8(Xt, 4 * c0 + i, 32)) = bf16_bits(xr[i]);
-                    else *reinterpret_cast<float*>(t8(Xt, 4 * c0 + i, 32)) = xr[i];
-                }
+                for (int i = 0; i < 4 * NCH; ++i) *reinterpret_cast<unsigned short*>(t8(Xt, 4 * c0 + i, 32)) = bf16_bits(xr[i]);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp no longer reads the X tile
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp no longer reads the X tile
             mbar_wait(bar_mma, gt & 1u);
             tc_fence_after();
             float mk[32];                                      // ReLU'(z_u) w2_u of this row (eq. 7 factor, old W2)
@@ -314,10 +315,23 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                     for (int c = 0; c + o < NSL; c += 2 * o) ypc[c] += ypc[c + o];
                 const float d = frow < vt ? scale * (ypc[0] - ycur) : 0.f;
                 if (hb == 0) Ds[frow] = d;
+                if constexpr (BF16) {
 #pragma unroll
-                for (int u = 0; u < 32; ++u) {                 // dZ1^T[u][row]: A operand of eq. 8
-                    if constexpr (BF16) *reinterpret_cast<unsigned short*>(t8(At, uoff + u, 64)) = bf16_bits(d * mk[u]);
-                    else *reinterpret_cast<float*>(t8(At, uoff + u, 64)) = d * mk[u];
+                    for (int u = 0; u < 32; ++u)               // dZ1^T[u][row]: A operand of eq. 8, K-major
+                        *reinterpret_cast<unsigned short*>(t8(At, uoff + u, 64)) = bf16_bits(d * mk[u]);
+                } else {
+                    // this row of dZ1 (32 units = 128 bytes): A operand of eq. 8, MN-major.  Rows r and r + 4 share a
+                    // swizzle phase, so they store the two 16-byte halves of a 32-byte chunk in opposite order: the 8 rows
+                    // of a quarter-warp then hit 8 different bank groups (no conflict) at the price of 4 selects per store
+                    const bool flip = (frow >> 2) & 1;
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const int g = c >> 1, h0 = c & 1;      // logical chunk, half taken by the rows that do not flip
+                        const float4 lo = make_float4(d * mk[8 * g], d * mk[8 * g + 1], d * mk[8 * g + 2], d * mk[8 * g + 3]);
+                        const float4 hi = make_float4(d * mk[8 * g + 4], d * mk[8 * g + 5], d * mk[8 * g + 6], d * mk[8 * g + 7]);
+                        const bool hsel = (h0 != 0) != flip;   // which half this thread stores now
+                        *reinterpret_cast<float4*>(At + hb * (BT * 128) + swz32(frow, g, hsel ? 1 : 0)) = hsel ? hi : lo;
+                    }
                 }
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // At, Xt (generic writes) -> MMA
@@ -326,17 +340,24 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
             if (warp == 0) {
                 tc_fence_after();
                 if (elect_one()) {
+                    if constexpr (BF16) {
 #pragma unroll
-                    for (int a = 0; a < NA; ++a) {
-                        const uint64_t adesc = smem_desc_sw128(smem_u32(At) + a * (64 * 128));
-                        const uint64_t bdesc = smem_desc_sw128(smem_u32(Xt) + a * (32 * 128));
+                        for (int a = 0; a < NA; ++a) {
+                            const uint64_t adesc = smem_desc_sw128(smem_u32(At) + a * (64 * 128));
+                            const uint64_t bdesc = smem_desc_sw128(smem_u32(Xt) + a * (32 * 128));
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
-                            if constexpr (BF16) mma_f16(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
-                            else mma_tf32(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
+                            for (int k = 0; k < 4; ++k) mma_f16(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
                         }
+                    } else {
+                        // both operands MN-major: 8 tile rows (1,024 bytes) per MMA; A = the two 32-unit planes of dZ1
+                        const uint64_t adesc = smem_desc_sw128_a32(smem_u32(At), BT * 128);
+                        const uint64_t bdesc = smem_desc_sw128_a32(smem_u32(Xs) + xst * kXBytes, 1024);
+#pragma unroll
+                        for (int k = 0; k < BT / 8; ++k)
+                            mma_tf32(tmem_base + 64, adesc + 64 * k, bdesc + 64 * k, idesc8 | kIdescAMajorMN | kIdescBMajorMN, (j | k) != 0);
                     }
                     tc_commit(bar_mma2);
+                    if constexpr (!BF16) tc_commit(bar_empty + 8 * xst);   // the tensor core was the only reader of the X tile
                 }
                 __syncwarp();
             }
@@ -421,7 +442,7 @@ cudaError_t launch_one(const float* X, int64_t n, const TcParams& p, cudaStream_
     static_assert(P::BYTES <= 227 * 1024, "shared-memory plan exceeds the per-CTA limit");
     if (n > 0x7fffffffLL - P::BT) return cudaErrorInvalidValue;          // TMA coordinates are int32
     alignas(64) CUtensorMap tmap;
-    if (!make_x_tensormap(&tmap, X, n, P::BT)) return cudaErrorNotSupported;
+    if (!make_x_tensormap(&tmap, X, n, P::BT, /*atom32=*/!BF16)) return cudaErrorNotSupported;
     auto kern = k_train_tc<C, S, BF16>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::BYTES);
     if (e != cudaSuccess) return e;
