@@ -60,6 +60,11 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
 }
 
+// MN-major 16-bit operand in the same layout (rows = K index, the 128 bytes of a row = 64 M or N elements; groups of 8 K rows,
+// 1,024 bytes apart; +2,048 bytes (16 rows) per K = 16; instruction-descriptor bit 15 (A) / 16 (B)): measured with a probe kernel
+__device__ __forceinline__ uint64_t smem_desc_sw128_mn16(uint32_t saddr) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (64ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+}
 // The same tile geometry with the "128-byte swizzle, 32-byte atom" (CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B; UMMA layout type 1):
 // the 32-byte chunk index is XORed with (row & 3), the pattern repeats every 4 rows (512 bytes).  It is the layout in which
 // a TF32 operand can be read in EITHER orientation (measured with a probe kernel, profiles/r02_microbench.md section 4):

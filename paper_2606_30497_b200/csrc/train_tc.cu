@@ -67,9 +67,9 @@ struct TcPlan {
     static constexpr uint32_t oX = 0;                                   // [kRing][BT][128 B]  A of eq. 1 (TF32)
     static constexpr uint32_t oXb = oX + kRing * XBYTES;                // [BT][128 B]         A of eq. 1 (BF16 copy)
     static constexpr uint32_t oW = oXb + (BF16 ? XBYTES : 0);           // [S][128 B]          B of eq. 1
-    static constexpr uint32_t oAt = oW + S * 128;                       // A of eq. 8 (dZ1^T): BF16 [NA][64][128 B] K-major; TF32 [2][BT][128 B] MN-major
-    static constexpr uint32_t oXt = oAt + (BF16 ? NA * 64 * 128 : BT * 256);                     // B of eq. 8 (X^T): BF16 [NA][32][128 B]; TF32: the X tile itself, MN-major
-    static constexpr uint32_t oH = oXt + (BF16 ? NA * 32 * 128 : 0);    // [NTH][BT][128 B]    H = ReLU(Z1)
+    static constexpr uint32_t oAt = oW + S * 128;                       // A of eq. 8 (dZ1 rows, MN-major): BF16 [BT][64 units x 2 B]; TF32 [2 planes][BT][32 units x 4 B]
+    static constexpr uint32_t oXt = oAt + (BF16 ? BT * 128 : BT * 256);                     // (end of At; B of eq. 8 is the X tile itself, MN-major: the BF16 copy or the landed TF32 tile)
+    static constexpr uint32_t oH = oXt;                                 // [NTH][BT][128 B]    H = ReLU(Z1)
     static constexpr uint32_t oYp = oH + NTH * BT * 128;                // [2][NSL][BT] floats
     static constexpr uint32_t oP2 = oYp + 2 * NSL * BT * 4;             // [kWarps][32] dW2 partials
     static constexpr uint32_t oW2 = oP2 + kWarps * 32 * 4;              // [S]
@@ -100,7 +100,6 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     unsigned char* Xb = smem + P::oXb;
     unsigned char* Wop = smem + P::oW;
     unsigned char* At = smem + P::oAt;
-    unsigned char* Xt = smem + P::oXt;
     unsigned char* Hs = smem + P::oH;
     float* ypp = reinterpret_cast<float*>(smem + P::oYp);
     float* part2 = reinterpret_cast<float*>(smem + P::oP2);
@@ -141,6 +140,8 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     // ---- one-time setup ---------------------------------------------------------------------------
     if (wowner) store_wop();
     for (int f = tid; f < (int)(P::oXt - P::oAt) / 4; f += kThreads) reinterpret_cast<float*>(At)[f] = 0.f;   // padding rows / plane stay 0
+    if constexpr (BF16)                                                   // the unused half of every row of the BF16 tile copy (read as N = 32..63 by eq. 8)
+        for (int f = tid; f < BT * 32; f += kThreads) reinterpret_cast<float*>(Xb)[f] = 0.f;
     if (tid < S) W2s[tid] = p.W2[crank * S + tid];
     if (tid == 0) {
         for (int b = 0; b < kRing; ++b) { mbar_init(bar_full + 8 * b, 1); mbar_init(bar_empty + 8 * b, BF16 ? kWarps : 1); }
@@ -190,14 +191,8 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     // instruction descriptors: D=f32, both operands K-major; eq. 1: M=128, N=32 (two chains) or 64; eq. 8: M=64, N=32
     constexpr uint32_t kFmt = BF16 ? 1u : 2u;
     constexpr uint32_t idesc1 = mma_idesc(kFmt, 128, S == 32 ? 32 : 64);
-    constexpr uint32_t idesc8 = mma_idesc(kFmt, 64, kIn);
+    constexpr uint32_t idesc8 = mma_idesc(kFmt, 64, BF16 ? 64 : kIn);   // BF16: N = 64, the width of a row of the BF16 tile copy
     constexpr int KS1 = BF16 ? 2 : 4;                          // MMAs per chain of eq. 1 (K = 16 or 8 each)
-    // position of (row r of the tile, operand row c) in the K-major operands of eq. 8: atom r/KA, k = r%KA
-    const int ka = BF16 ? frow >> 6 : frow >> 5, kk = BF16 ? frow & 63 : frow & 31;
-    auto t8 = [&](unsigned char* base, int orow, int rows_per_atom) -> unsigned char* {   // address of element (orow, k = frow)
-        return BF16 ? base + ka * (rows_per_atom * 128) + swz(orow, kk >> 3) + (kk & 7) * 2
-                    : base + ka * (rows_per_atom * 128) + swz(orow, kk >> 2) + (kk & 3) * 4;
-    };
     constexpr int NCH = 8 / NTH;                               // 16-byte chunks of an X row this thread handles
     const int c0 = NTH == 2 ? hb * 4 : 0;
     unsigned gt = 0;
@@ -255,7 +250,7 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 }
             };
             if constexpr (!BF16) issue_eq1();                  // TF32: the tile is the operand as TMA delivered it
-            // BF16: this thread's part of its X row: rounded copy for eq. 1, transposed into the B operand of eq. 8
+            // BF16: this thread's part of its X row, rounded into the BF16 copy of the tile (A of eq. 1 K-major, B of eq. 8 MN-major)
             // (TF32: the tile is read by the tensor core only, in both orientations; eq. 8's commit releases the slot)
             if constexpr (BF16) {
                 float xr[4 * NCH];
@@ -270,8 +265,6 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncthreads();                           // every row of the BF16 copy is written
                 issue_eq1();
-#pragma unroll
-                for (int i = 0; i < 4 * NCH; ++i) *reinterpret_cast<unsigned short*>(t8(Xt, 4 * c0 + i, 32)) = bf16_bits(xr[i]);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_empty + 8 * xst);   // this warp no longer reads the X tile
             }
@@ -316,9 +309,12 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 const float d = frow < vt ? scale * (ypc[0] - ycur) : 0.f;
                 if (hb == 0) Ds[frow] = d;
                 if constexpr (BF16) {
+                    float dz[32];
 #pragma unroll
-                    for (int u = 0; u < 32; ++u)               // dZ1^T[u][row]: A operand of eq. 8, K-major
-                        *reinterpret_cast<unsigned short*>(t8(At, uoff + u, 64)) = bf16_bits(d * mk[u]);
+                    for (int u = 0; u < 32; ++u) dz[u] = d * mk[u];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)                // this row of dZ1 (64 units x 2 B = 128 bytes; S = 32: the upper half stays 0)
+                        *reinterpret_cast<uint4*>(At + swz(frow, 4 * hb + c)) = pack_bf16x8(dz + 8 * c);
                 } else {
                     // this row of dZ1 (32 units = 128 bytes): A operand of eq. 8, MN-major.  Rows r and r + 4 share a
                     // swizzle phase, so they store the two 16-byte halves of a 32-byte chunk in opposite order: the 8 rows
@@ -334,20 +330,19 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                     }
                 }
             }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // At, Xt (generic writes) -> MMA
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // At (generic writes) -> MMA
             __syncthreads();
             // ---------------- eq. 8 on the tensor cores: dW1^T += dZ1^T X ----------------
             if (warp == 0) {
                 tc_fence_after();
                 if (elect_one()) {
                     if constexpr (BF16) {
+                        // both operands MN-major, 16 tile rows (2,048 bytes) per MMA; B = the BF16 copy of the tile, whose rows are
+                        // 64 elements wide (N = 64: the upper 32 columns are zeros and their results are never read)
+                        const uint64_t adesc = smem_desc_sw128_mn16(smem_u32(At)), bdesc = smem_desc_sw128_mn16(smem_u32(Xb));
 #pragma unroll
-                        for (int a = 0; a < NA; ++a) {
-                            const uint64_t adesc = smem_desc_sw128(smem_u32(At) + a * (64 * 128));
-                            const uint64_t bdesc = smem_desc_sw128(smem_u32(Xt) + a * (32 * 128));
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) mma_f16(tmem_base + 64, adesc + 2 * k, bdesc + 2 * k, idesc8, (j | a | k) != 0);
-                        }
+                        for (int k = 0; k < BT / 16; ++k)
+                            mma_f16(tmem_base + 64, adesc + 128 * k, bdesc + 128 * k, idesc8 | kIdescAMajorMN | kIdescBMajorMN, (j | k) != 0);
                     } else {
                         // both operands MN-major: 8 tile rows (1,024 bytes) per MMA; A = the two 32-unit planes of dZ1
                         const uint64_t adesc = smem_desc_sw128_a32(smem_u32(At), BT * 128);
@@ -374,7 +369,7 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 g2 += (gp[0] + gp[1]) + (gp[2] + gp[3]);
             }
             ycur = ynext;
-            mbar_wait(bar_mma2, gt & 1u);                      // eq. 8 of this tile has read At / Xt
+            mbar_wait(bar_mma2, gt & 1u);                      // eq. 8 of this tile has read At and the tile
             tc_fence_after();
             __syncthreads();                                   // and every warp is done with Hs / Ds
         }
