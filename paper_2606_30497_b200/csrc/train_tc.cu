@@ -191,7 +191,7 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     // instruction descriptors: D=f32, both operands K-major; eq. 1: M=128, N=32 (two chains) or 64; eq. 8: M=64, N=32
     constexpr uint32_t kFmt = BF16 ? 1u : 2u;
     constexpr uint32_t idesc1 = mma_idesc(kFmt, 128, S == 32 ? 32 : 64);
-    constexpr uint32_t idesc8 = mma_idesc(kFmt, 64, BF16 ? 64 : kIn);   // BF16: N = 64, the width of a row of the BF16 tile copy
+    constexpr uint32_t idesc8 = mma_idesc(kFmt, 64, kIn);
     constexpr int KS1 = BF16 ? 2 : 4;                          // MMAs per chain of eq. 1 (K = 16 or 8 each)
     constexpr int NCH = 8 / NTH;                               // 16-byte chunks of an X row this thread handles
     const int c0 = NTH == 2 ? hb * 4 : 0;
@@ -337,8 +337,8 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                 tc_fence_after();
                 if (elect_one()) {
                     if constexpr (BF16) {
-                        // both operands MN-major, 16 tile rows (2,048 bytes) per MMA; B = the BF16 copy of the tile, whose rows are
-                        // 64 elements wide (N = 64: the upper 32 columns are zeros and their results are never read)
+                        // both operands MN-major, 16 tile rows (2,048 bytes) per MMA; B = the BF16 copy of the tile (N = 32: the first
+                        // 64 bytes of its 128-byte rows)
                         const uint64_t adesc = smem_desc_sw128_mn16(smem_u32(At)), bdesc = smem_desc_sw128_mn16(smem_u32(Xb));
 #pragma unroll
                         for (int k = 0; k < BT / 16; ++k)
