@@ -163,20 +163,23 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     const long long total = p.total_steps;
     int seq = 0;
     unsigned long long bad_order = 0;     // batch_order entries outside [0, nb): clamped, counted, reported
-    auto batch_index = [&](long long step, int sq) -> int {
+    // The table entry of step k is loaded when step k-3 starts and only looked at (range check) when step k-2
+    // starts, so the global-load latency never sits on a step's critical path (as in train_fused.cu).
+    auto checked = [&](int t, int sq) -> int {
         if (!p.order) return sq;
-        const int t = __ldg(p.order + step);
         if ((unsigned)t < (unsigned)p.nbi) return t;
         ++bad_order;
         return t < 0 ? 0 : p.nbi - 1;
     };
+    auto raw_entry = [&](long long step) -> int { return (p.order && step < total) ? __ldg(p.order + step) : 0; };
     auto rows_of = [&](int t) -> int { return t == p.nbi - 1 ? p.m_last : p.B; };
     auto issue_tile = [&](long long g0, unsigned nbuf) {      // one thread; the box is always BT rows
         mbar_arrive_expect_tx(bar_full + 8 * nbuf, kXBytes);  // rows past n are zero-filled, still counted
         tma_load_2d(smem_u32(Xs) + nbuf * kXBytes, &tmapX, 0, (int)g0, bar_full + 8 * nbuf);
     };
-    int t_cur = batch_index(0, 0);
-    int t_next = total > 1 ? batch_index(1, 1 % p.nbi) : 0;
+    int t_cur = checked(raw_entry(0), 0);
+    int t_next = total > 1 ? checked(raw_entry(1), 1 % p.nbi) : 0;
+    int raw2 = raw_entry(2);                          // entry of step + 2, not yet checked
     seq = 2 % p.nbi;
     if (tid == 0) issue_tile((long long)t_cur * p.B, 0);
 
@@ -197,7 +200,8 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     const int c0 = NTH == 2 ? hb * 4 : 0;
     unsigned gt = 0;
     for (long long step = 0; step < total; ++step) {
-        const int t_nn = (step + 2 < total) ? batch_index(step + 2, seq) : 0;
+        const int t_nn = (step + 2 < total) ? checked(raw2, seq) : 0;
+        raw2 = raw_entry(step + 3);
         seq = seq + 1 == p.nbi ? 0 : seq + 1;
         const long long r0 = (long long)t_cur * p.B;
         const int m = rows_of(t_cur);
