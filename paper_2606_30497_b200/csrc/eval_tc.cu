@@ -226,7 +226,6 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
             // ... and converter: tile i is converted as soon as it has landed; the slot of tile i - 1 is refilled
             // afterwards (its MMA has had a whole conversion to finish), so the two duties never wait on each other
             for (uint32_t i = 0; i < nt; ++i) {
-                const uint32_t st = i % NST;
                 convert_half(i, 0);
                 if (i >= 1 && i - 1 + NST < nt) refill(i - 1 + NST);
             }

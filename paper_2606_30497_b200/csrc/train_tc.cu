@@ -59,9 +59,6 @@ template <int C, int S, bool BF16>
 struct TcPlan {
     static constexpr int NTH = S / 32;                 // threads per row
     static constexpr int BT = 256 / NTH;               // rows per tile
-    static constexpr int EB = BF16 ? 2 : 4;            // operand element bytes
-    static constexpr int KA = 128 / EB;                // rows (K elements) per 128-byte swizzle atom of eq. 8
-    static constexpr int NA = BT / KA;                 // K atoms of eq. 8
     static constexpr int NSL = C * NTH;                // Ypred partial slots per row
     static constexpr uint32_t XBYTES = BT * 128;       // one X tile
     static constexpr uint32_t oX = 0;                                   // [kRing][BT][128 B]  A of eq. 1 (TF32)
@@ -83,17 +80,12 @@ struct TcPlan {
 __device__ __forceinline__ uint4 pack_bf16x8(const float* v) {
     return make_uint4(bf16x2(v[0], v[1]), bf16x2(v[2], v[3]), bf16x2(v[4], v[5]), bf16x2(v[6], v[7]));
 }
-__device__ __forceinline__ unsigned short bf16_bits(float v) {
-    unsigned short r;
-    asm("cvt.rn.bf16.f32 %0, %1;" : "=h"(r) : "f"(v));
-    return r;
-}
 
 template <int C, int S, bool BF16>
 __global__ void __launch_bounds__(kThreads, 1)
 k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     using P = TcPlan<C, S, BF16>;
-    constexpr int NTH = P::NTH, BT = P::BT, NA = P::NA, NSL = P::NSL;
+    constexpr int NTH = P::NTH, BT = P::BT, NSL = P::NSL;
     constexpr uint32_t kXBytes = P::XBYTES;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* Xs = smem + P::oX;
