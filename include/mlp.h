@@ -155,6 +155,23 @@ int mlp_eval_loss_ws(const float* X, const float* Y, int64_t n, const float* W1,
                      double* d_out, int variant, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * mlp_eval_loss_static -- mlp_eval_loss_async for callers that cannot allocate device memory (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same kernels,
+ * arguments, variants, results and error behaviour as mlp_eval_loss_async; the per-CTA partial sums
+ * and the last-block ticket live in a file-scope __device__ array of the library (8,448 bytes, held
+ * by every GPU that loads the library until the process exits) instead of a pool slot.  The call
+ * makes no cudaMalloc / cudaFree and creates no events or streams.  The array holds
+ * MLP_STATIC_EVAL_MAX_CTAS partial sums; a launch that needs more (one CTA per SM: a device with
+ * more SMs than that) returns MLP_ERR_UNSUPPORTED.  ALL calls on a device share the one array:
+ * each call clears the ticket on `stream` before its kernel, and two calls whose kernels may
+ * overlap on the GPU (different streams without an ordering between them) race -- order them, or
+ * use mlp_eval_loss_async / mlp_eval_loss_ws for the concurrent ones.  Calls on one stream are safe.
+ */
+#define MLP_STATIC_EVAL_MAX_CTAS 1024
+int mlp_eval_loss_static(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+                         double* d_out, int variant, void* stream);
+
+/*
  * Host-buffer entry points (end-to-end path): copy X/Y (and weights / order) from HOST memory
  * to library-owned device buffers, run the same kernels, copy the result back, synchronise.
  * W1_host/W2_host are read and overwritten with the trained weights.  order_host may be NULL; if

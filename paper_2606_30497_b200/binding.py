@@ -25,7 +25,7 @@ VARIANT_TF32X3 = 6
 
 EXPORTS = [
     "mlp_init", "mlp_init_weights", "mlp_train", "mlp_train_ex", "mlp_eval_loss",
-    "mlp_eval_loss_async", "mlp_eval_loss_ws", "mlp_eval_workspace_bytes", "mlp_train_host", "mlp_fit_host",
+    "mlp_eval_loss_async", "mlp_eval_loss_static", "mlp_eval_loss_ws", "mlp_eval_workspace_bytes", "mlp_train_host", "mlp_fit_host",
     "mlp_eval_loss_host", "mlp_set_cluster", "mlp_train_rows", "mlp_get_cluster", "mlp_get_cluster_for",
     "mlp_get_train_stats", "mlp_train_order_errors", "mlp_launch_count", "mlp_last_error", "mlp_version",
     "mlp_shutdown",
@@ -60,6 +60,8 @@ def lib():
     L.mlp_eval_loss.argtypes = [vp, vp, i64, vp, vp, vp]; L.mlp_eval_loss.restype = f64
     L.mlp_eval_loss_async.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp]
     L.mlp_eval_loss_async.restype = i32
+    L.mlp_eval_loss_static.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp]
+    L.mlp_eval_loss_static.restype = i32
     L.mlp_eval_loss_ws.argtypes = [vp, vp, i64, vp, vp, vp, i32, vp, C.c_size_t, vp]
     L.mlp_eval_loss_ws.restype = i32
     L.mlp_eval_workspace_bytes.argtypes = []; L.mlp_eval_workspace_bytes.restype = C.c_size_t
@@ -144,6 +146,12 @@ def mlp_eval_loss_async(X, Y, n, W1, W2, d_out, variant=VARIANT_FUSED, stream=No
     _check(lib().mlp_eval_loss_async(_dptr(X, "float32", "X"), _dptr(Y, "float32", "Y"), int(n),
                                      _dptr(W1, "float32", "W1"), _dptr(W2, "float32", "W2"),
                                      _dptr(d_out, "float64", "d_out"), int(variant), _stream(stream)))
+
+
+def mlp_eval_loss_static(X, Y, n, W1, W2, d_out, variant=VARIANT_FUSED, stream=None) -> None:
+    _check(lib().mlp_eval_loss_static(_dptr(X, "float32", "X"), _dptr(Y, "float32", "Y"), int(n),
+                                      _dptr(W1, "float32", "W1"), _dptr(W2, "float32", "W2"),
+                                      _dptr(d_out, "float64", "d_out"), int(variant), _stream(stream)))
 
 
 def mlp_eval_workspace_bytes() -> int:

@@ -13,6 +13,13 @@
 #include "../../include/mlp.h"
 #include "internal.h"
 
+// Scratch of mlp_eval_loss_static (include/mlp.h): per-CTA partial sums [0, MLP_STATIC_EVAL_MAX_CTAS), then
+// the last-block ticket.  File scope, so every GPU that loads this library holds these bytes until exit.  In
+// host code this name is only a stand-in for the symbol: the device address comes from cudaGetSymbolAddress
+// (static_eval_scratch below), once per device.
+constexpr int kStaticEvalDoubles = MLP_STATIC_EVAL_MAX_CTAS + 32;           // 8,448 bytes
+static __device__ __align__(256) double g_static_eval_scratch[kStaticEvalDoubles];
+
 namespace {
 
 using namespace mlp;
@@ -331,6 +338,26 @@ int check_host_train_args(const float* X_host, const float* Y_host, int64_t n, i
     return MLP_OK;
 }
 
+// Device address of g_static_eval_scratch and the SM count of the CURRENT device, looked up once per device.
+constexpr int kMaxDevices = 64;
+double* g_static_ptr[kMaxDevices] = {};
+int g_static_sms[kMaxDevices] = {};
+
+int static_eval_scratch(double** ptr, int* sms) {
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(MLP_ERR_UNSUPPORTED, "device ordinal %d is outside [0, %d)", dev, kMaxDevices);
+    if (!g_static_ptr[dev]) {
+        double* p = nullptr;
+        CK(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_eval_scratch));
+        CK(cudaDeviceGetAttribute(&g_static_sms[dev], cudaDevAttrMultiProcessorCount, dev));
+        g_static_ptr[dev] = p;
+    }
+    *ptr = g_static_ptr[dev];
+    *sms = g_static_sms[dev];
+    return MLP_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -409,6 +436,34 @@ int mlp_eval_loss_ws(const float* X, const float* Y, int64_t n, const float* W1,
     ws.result = ws.partials + g.num_sms + 1;
     ws.slot = -1;
     return eval_launch(X, Y, n, W1, W2, d_out, variant, ws, (cudaStream_t)stream);
+}
+
+int mlp_eval_loss_static(const float* X, const float* Y, int64_t n, const float* W1, const float* W2,
+                         double* d_out, int variant, void* stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!d_out) return fail(MLP_ERR_BAD_ARG, "NULL pointer argument");
+    int rc = check_eval_args(X, Y, n, W1, W2, variant);
+    if (rc) return rc;
+    double* scratch = nullptr;
+    int sms = 0;
+    if ((rc = static_eval_scratch(&scratch, &sms))) return rc;
+    const int grid = variant == MLP_VARIANT_FUSED ? eval_fp32_grid(g.hidden, sms) : sms;   // one partial sum per CTA
+    if (grid > MLP_STATIC_EVAL_MAX_CTAS)
+        return fail(MLP_ERR_UNSUPPORTED, "this launch needs %d per-CTA partial sums, the static scratch holds %d "
+                    "(MLP_STATIC_EVAL_MAX_CTAS); use mlp_eval_loss_async or mlp_eval_loss_ws", grid,
+                    MLP_STATIC_EVAL_MAX_CTAS);
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned int* ticket = reinterpret_cast<unsigned int*>(scratch + MLP_STATIC_EVAL_MAX_CTAS);
+    // the array keeps what the last call left: the ticket must start at zero, the partial sums are
+    // all overwritten before they are read
+    CK(cudaMemsetAsync(ticket, 0, sizeof(double), st));
+    cudaError_t e;
+    if (variant == MLP_VARIANT_FUSED)
+        e = launch_eval_fp32(X, Y, n, W1, W2, g.hidden, scratch, ticket, grid, d_out, st, &g.launches);
+    else
+        e = launch_eval_tc(X, Y, n, W1, W2, g.hidden, variant, scratch, ticket, grid, d_out, st, &g.launches);
+    if (e != cudaSuccess) return cuda_fail(e, "eval kernel launch");
+    return MLP_OK;
 }
 
 int mlp_train_rows(const float* X, const float* Y, int64_t n, int batch, float lr, int epochs,
