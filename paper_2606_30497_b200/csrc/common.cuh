@@ -100,6 +100,16 @@ __device__ __forceinline__ void st_async_f32(uint32_t raddr, float v, uint32_t r
                  ::"r"(raddr), "r"(__float_as_uint(v)), "r"(rbar));   // register operands only:
     // no "memory" clobber, so independent shared-memory loads may be scheduled across it
 }
+// the same with 8 / 16 bytes (the destination must be aligned to the size)
+__device__ __forceinline__ void st_async_v2(uint32_t raddr, float a, float b, uint32_t rbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b32 [%0], {%1, %2}, [%3];"
+                 ::"r"(raddr), "r"(__float_as_uint(a)), "r"(__float_as_uint(b)), "r"(rbar));
+}
+__device__ __forceinline__ void st_async_v4(uint32_t raddr, float a, float b, float c, float d, uint32_t rbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(raddr), "r"(__float_as_uint(a)), "r"(__float_as_uint(b)), "r"(__float_as_uint(c)),
+                   "r"(__float_as_uint(d)), "r"(rbar));
+}
 __device__ __forceinline__ void cluster_arrive() {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
 }

@@ -20,8 +20,11 @@
 //   * per-row partial Ypred: transposing shuffle tree over the LPS lanes, then pushed to every CTA
 //     of the cluster with st.async (DSMEM store that completes transaction bytes on the
 //     destination's mbarrier: one hop, no flag), one fixed peer per lane, straight-line code (the
-//     cluster size is a template parameter).  The tile is processed as NSPLIT row groups so that
-//     the exchange of one group is in flight while the other group computes;
+//     cluster size is a template parameter).  A store carries the totals of up to four consecutive
+//     rows (st.async .v4 / .v2): a quarter of the remote stores and of the barrier updates of
+//     per-row stores, which is what the exchange of a 16-CTA cluster was bound by.  The tile is
+//     processed as NSPLIT row groups so that the exchange of one group is in flight while the
+//     other group computes;
 //   * backward (eqs. 5-8), K-split over the sub-groups: every CTA sums the C partials (fixed tree)
 //     -> dZ2; the lane of sub-group s accumulates dW1 only for inputs [IPS*s, IPS*(s+1)) of its four
 //     units (32 registers at SPW = 4) but over the rows of ALL sub-groups, whose dZ1 arrives by
@@ -169,10 +172,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
 
     const int rowl = warp * ITER;                     // first row of this lane inside its block
     // Ypred exchange: every lane pushes to one fixed peer (staggered by rank)
-    constexpr int RPI = 32 / C;                       // rows served per push iteration (C <= 32)
+    constexpr int RPI = 32 / C;                       // segments served per push iteration (C <= 32)
     const uint32_t pd = ((lane & (C - 1)) + crank) & (C - 1);
     const uint32_t rem_ypp = mapa(smem_u32(ypp), pd), rem_bar = mapa(bar_yp, pd);
-    constexpr int NPUSH = (ITS * SPW * C + 31) / 32;
+    constexpr int VW = ITS >= 4 ? 4 : ITS;            // rows per remote store (st.async .v4 / .v2 / scalar)
+    constexpr int NSEG = ITS * SPW / VW;              // VW-row segments of a warp's exchange sub-tile
+    constexpr int NPUSH = (NSEG * C + 31) / 32;
     float* mypart = part + warp * (S * kIn);
     // Targets: lane l < ITER*SPW of a warp holds Y of the warp's row (l / ITER, l % ITER); it is
     // fetched one tile ahead (global-load latency hidden by a whole tile) and handed to the lane
@@ -309,17 +314,23 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                         }
                     }
                     GroupReduce<ITS, LPS, 1, LSH>::run(pv, lu);
-                    // push: lane l serves ONE destination CTA (pd) and the rows l/C, l/C + 32/C, ...
-                    // of the warp's ITS*SPW totals, fetched from their holder lanes by shuffle
+                    // push: lane l serves ONE destination CTA (pd) and the segments l/C, l/C + 32/C, ... of the
+                    // warp's NSEG segments (VW consecutive rows of one sub-group), whose totals it fetches from
+                    // their holder lanes by shuffle and sends as one 4*VW-byte store
 #pragma unroll
                     for (int i = 0; i < NPUSH; ++i) {
-                        const int r = lane / C + i * RPI;
-                        const int sp = r / ITS, k = r % ITS;
-                        const float v = __shfl_sync(0xffffffffu, pv[0], lane_of(sp, k) & 31);
-                        if (r < ITS * SPW) {
-                            const int row = sp * RB + rowl + q * ITS + k;
-                            st_async_f32(rem_ypp + (buf * (C * BTP) + crank * BTP + row + sp * PADR) * 4, v,
-                                         rem_bar + 8 * (buf * NSPLIT + q));
+                        const int r = lane / C + i * RPI;          // segment: VW consecutive rows of sub-group sp
+                        const int sp = r / (ITS / VW), k0 = (r % (ITS / VW)) * VW;
+                        float v[VW];
+#pragma unroll
+                        for (int k = 0; k < VW; ++k) v[k] = __shfl_sync(0xffffffffu, pv[0], lane_of(sp, k0 + k) & 31);
+                        if (r < NSEG) {
+                            const int row = sp * RB + rowl + q * ITS + k0;
+                            const uint32_t dst = rem_ypp + (buf * (C * BTP) + crank * BTP + row + sp * PADR) * 4;
+                            const uint32_t rb = rem_bar + 8 * (buf * NSPLIT + q);
+                            if constexpr (VW == 4) st_async_v4(dst, v[0], v[1], v[2], v[3], rb);
+                            else if constexpr (VW == 2) st_async_v2(dst, v[0], v[1], rb);
+                            else st_async_f32(dst, v[0], rb);
                         }
                     }
                 }
