@@ -111,6 +111,13 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
         }
     }
     __syncwarp();
+    // the warp's first group: its W1 column loads are issued together with the W2 loads of the sign count, so
+    // the two global round trips (cold after a flush of L2) overlap
+    float wcol[kIn];
+    if (warp < NG) {
+#pragma unroll
+        for (int k = 0; k < kIn; ++k) wcol[k] = __ldg(W1 + (size_t)k * H + warp * 32 + lane);
+    }
     for (int g = warp; g < NG; g += NW) {                      // a warp per group of 32 hidden units
         const unsigned bal = __ballot_sync(0xffffffffu, __ldg(W2 + g * 32 + lane) >= 0.f);
         if (lane == 0) wcnt[g] = __popc(bal);
@@ -119,9 +126,10 @@ k_eval_tc(const __grid_constant__ CUtensorMap tmapX, const float* __restrict__ Y
     for (int g = warp; g < NG; g += NW) {
         const int j0 = g * 32 + lane;
         // lane stages column j0 of W1: 32 independent coalesced loads in flight at once
-        float wcol[kIn];
+        if (g != warp) {
 #pragma unroll
-        for (int k = 0; k < kIn; ++k) wcol[k] = __ldg(W1 + (size_t)k * H + j0);
+            for (int k = 0; k < kIn; ++k) wcol[k] = __ldg(W1 + (size_t)k * H + j0);
+        }
         const float w2v = __ldg(W2 + j0);
         const unsigned bal = __ballot_sync(0xffffffffu, w2v >= 0.f);
         int before = __popc(bal & ((1u << lane) - 1u)), total = 0;
