@@ -89,3 +89,30 @@ def test_static_eval_allocates_nothing_and_validates():
     B.mlp_init(2, 32, 512, 1)
     with pytest.raises(B.MlpError):
         B.mlp_eval_loss_static(dX, dY, n, d1, d2, out[0:1], B.VARIANT_TF32X3)     # hidden > 256
+
+
+def test_static_eval_under_graph_capture():
+    """The motivating use: after one warm-up call (symbol lookup, module load), the call is captured into a CUDA
+    graph (stream capture forbids cudaMalloc) and replayed; every replay equals mlp_eval_loss_async bit for bit."""
+    B.mlp_init(2, 32, 128, 1)
+    n = 50001
+    X, Y = datagen.make_dataset(n, 0.1, seed_x=61)
+    W1, W2 = O.init_weights(4, 32, 128)
+    dX, dY, d1, d2 = dev(X), dev(Y), dev(W1), dev(W2)
+    want = torch.zeros(2, dtype=torch.float64, device="cuda")
+    B.mlp_eval_loss_async(dX, dY, n, d1, d2, want[0:1], B.VARIANT_FUSED)
+    B.mlp_eval_loss_async(dX, dY, n, d1, d2, want[1:2], B.VARIANT_TF32)
+    out = torch.zeros(2, dtype=torch.float64, device="cuda")
+    B.mlp_eval_loss_static(dX, dY, n, d1, d2, out[0:1], B.VARIANT_FUSED)        # warm-up, outside the capture
+    B.mlp_eval_loss_static(dX, dY, n, d1, d2, out[1:2], B.VARIANT_TF32)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        st = torch.cuda.current_stream()
+        B.mlp_eval_loss_static(dX, dY, n, d1, d2, out[0:1], B.VARIANT_FUSED, st)
+        B.mlp_eval_loss_static(dX, dY, n, d1, d2, out[1:2], B.VARIANT_TF32, st)
+    for _ in range(3):
+        out.fill_(-1.0)
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, want), (out.cpu().numpy(), want.cpu().numpy())
