@@ -273,9 +273,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_train_fused(const TrainParams p
                             w[rel][u][2 * c] = a.x; w[rel][u][2 * c + 1] = a.y;
                         }
                 };
+                // one-row tiles (batches <= 32 rows) are latency-bound: the first weight chunk is requested before
+                // the X tile is awaited (-3.5 % per step at B = 32; with more rows per lane it is a wash or a loss)
+                if constexpr (ITER == 1) load_w_chunk(0);
                 mbar_wait(bar_full + 8 * xst, xph);
                 const float* Xh = Xl + 16 * kh;              // this lane's half of its rows
-                load_w_chunk(0);
+                if constexpr (ITER > 1) load_w_chunk(0);
 #pragma unroll
                 for (int q = 0; q < NSPLIT; ++q) {
                     float pv[ITS];
