@@ -5,7 +5,9 @@
 // tensor cores (tcgen05.mma, fp32 accumulate in TMEM, fp32 master weights):
 //   eq. 1  Z1 = X W1        per tile chains of M=128 (rows), N=32 or 64 (units of this CTA), K=32;
 //   eq. 8  dW1^T = dZ1^T X  one chain M=64 (units), N=32 (inputs), K = rows of the tile, accumulated in
-//                           TMEM across the tiles of a batch.
+//                           TMEM across the tiles of a batch.  TF32 with 32 units per CTA: the two row halves
+//                           of the tile run side by side (M=64 = units x 2 halves, N=64 = inputs x 2 halves,
+//                           half as many MMAs) and the two diagonal blocks are summed at the end of the batch.
 // Operand precision: TF32 (kind::tf32: fp32 bits in shared memory, truncated by the tensor core) or BF16
 // (kind::f16: the threads round every operand to BF16, round to nearest even, as they stage it).
 // Everything else stays fp32 on the CUDA cores.
@@ -187,6 +189,10 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
     constexpr uint32_t kFmt = BF16 ? 1u : 2u;
     constexpr uint32_t idesc1 = mma_idesc(kFmt, 128, S == 32 ? 32 : 64);
     constexpr uint32_t idesc8 = mma_idesc(kFmt, 64, kIn);
+    // TF32, 32 units per CTA (one thread per tile row, BT = 256): eq. 8 folds the tile's two row halves side by side
+    // (see there), 16 MMAs of N = 64 instead of 32 of N = 32
+    constexpr bool FOLD = !BF16 && S == 32;
+    constexpr uint32_t idesc8f = mma_idesc(kFmt, 64, 2 * kIn);
     constexpr int KS1 = BF16 ? 2 : 4;                          // MMAs per chain of eq. 1 (K = 16 or 8 each)
     constexpr int NCH = 8 / NTH;                               // 16-byte chunks of an X row this thread handles
     const int c0 = NTH == 2 ? hb * 4 : 0;
@@ -340,12 +346,25 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
                         for (int k = 0; k < BT / 16; ++k)
                             mma_f16(tmem_base + 64, adesc + 128 * k, bdesc + 128 * k, idesc8 | kIdescAMajorMN | kIdescBMajorMN, (j | k) != 0);
                     } else {
+                        if constexpr (FOLD) {
+                            // the chain of tiny MMAs costs per instruction (~30 cycles each), so the two row halves of the tile
+                            // go through it side by side: A = [dZ1 rows k | dZ1 rows 128 + k] (M = 64: two 32-element column
+                            // blocks 16 KB apart in At), B = [X rows k | X rows 128 + k] (N = 64, likewise in the tile).  The
+                            // diagonal blocks of D (rows 0-31 x columns 0-31, rows 32-63 x columns 32-63) are the two halves
+                            // of dW1^T, summed in the epilogue; the off-diagonal blocks are not read.
+                            const uint64_t adesc = smem_desc_sw128_a32(smem_u32(At), 128 * 128);
+                            const uint64_t bdesc = smem_desc_sw128_a32(smem_u32(Xs) + xst * kXBytes, 128 * 128);
+#pragma unroll
+                            for (int k = 0; k < BT / 16; ++k)
+                                mma_tf32(tmem_base + 64, adesc + 64 * k, bdesc + 64 * k, idesc8f | kIdescAMajorMN | kIdescBMajorMN, (j | k) != 0);
+                        } else {
                         // both operands MN-major: 8 tile rows (1,024 bytes) per MMA; A = the two 32-unit planes of dZ1
                         const uint64_t adesc = smem_desc_sw128_a32(smem_u32(At), BT * 128);
                         const uint64_t bdesc = smem_desc_sw128_a32(smem_u32(Xs) + xst * kXBytes, 1024);
 #pragma unroll
                         for (int k = 0; k < BT / 8; ++k)
                             mma_tf32(tmem_base + 64, adesc + 64 * k, bdesc + 64 * k, idesc8 | kIdescAMajorMN | kIdescBMajorMN, (j | k) != 0);
+                        }
                     }
                     tc_commit(bar_mma2);
                     if constexpr (!BF16) tc_commit(bar_empty + 8 * xst);   // the tensor core was the only reader of the X tile
@@ -372,12 +391,40 @@ k_train_tc(const __grid_constant__ CUtensorMap tmapX, const TcParams p) {
 
         // ---------------- end of batch: eq. 9 ----------------
         part2[warp * 32 + lane] = g2;
+        if constexpr (FOLD) {
+            // second diagonal block of the folded eq. 8: accumulator rows 32-63 (lanes 0-15 of warps 2, 3), columns 32-63;
+            // handed to the owners of rows 0-31 through the (now idle) H buffer, 128-byte rows, chunks swizzled by lane
+            if (warp == 2 || warp == 3) {
+                uint32_t dh[32];
+                tmem_ld32(tdw + 32, dh);
+                tmem_ld_wait();
+                tc_fence_before();
+                if (lane < 16) {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c)
+                        *reinterpret_cast<uint4*>(Hs + ((warp - 2) * 16 + lane) * 128 + ((c ^ (lane & 7)) << 4)) =
+                            make_uint4(dh[4 * c], dh[4 * c + 1], dh[4 * c + 2], dh[4 * c + 3]);
+                }
+            }
+        }
         __syncthreads();
         if (warp < S / 16) {                                   // owners of the eq. 8 accumulator rows
             uint32_t dw[32];
             tmem_ld32(tdw, dw);
             tmem_ld_wait();
             tc_fence_before();
+            if constexpr (FOLD) {
+                if (wowner) {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const float4 v = *reinterpret_cast<const float4*>(Hs + wu * 128 + ((c ^ (lane & 7)) << 4));
+                        dw[4 * c] = __float_as_uint(__uint_as_float(dw[4 * c]) + v.x);
+                        dw[4 * c + 1] = __float_as_uint(__uint_as_float(dw[4 * c + 1]) + v.y);
+                        dw[4 * c + 2] = __float_as_uint(__uint_as_float(dw[4 * c + 2]) + v.z);
+                        dw[4 * c + 3] = __float_as_uint(__uint_as_float(dw[4 * c + 3]) + v.w);
+                    }
+                }
+            }
             if (wowner) {
 #pragma unroll
                 for (int i = 0; i < kIn; ++i) wrow[i] = fmaf(-p.lr, __uint_as_float(dw[i]), wrow[i]);   // W - lr*dW
