@@ -14,7 +14,7 @@
  *   - Pointers named X, Y, W1, W2, batch_order, d_out are DEVICE pointers owned by the caller
  *     (e.g. torch allocations); pointers with an `_host` suffix are HOST pointers.  The library
  *     never frees or retains caller memory.  Library-owned scratch is created lazily and
- *     released by mlp_shutdown().
+ *     released by mlp_shutdown() (mlp_eval_loss_static allocates nothing, see there).
  *   - Layout: all tensors fp32, row-major, dense: X [n x 32], Y [n], W1 [32 x hidden],
  *     W2 [hidden].  X must be 16-byte aligned, Y 4-byte aligned, W1 16-byte aligned.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
@@ -26,7 +26,9 @@
  *     workspace (per-CTA partial sums, ticket, result) from a library-owned pool of 32 slots, a slot
  *     being reused only after the launch that last used it has completed (the later stream is made
  *     to wait otherwise), and every fused training launch writes its statistics to its own slot
- *     (64 slots).  mlp_eval_loss_ws takes a caller-owned workspace instead.  The entry points
+ *     (64 slots).  mlp_eval_loss_ws takes a caller-owned workspace instead; mlp_eval_loss_static
+ *     uses ONE file-scope device array for all its calls, which therefore must not overlap on the
+ *     device (see there).  The entry points
  *     themselves are serialised by a mutex (enqueueing is cheap; the kernels run asynchronously).
  *   - There is no CPU fallback: without a CUDA device every compute entry returns MLP_ERR_CUDA.
  */
