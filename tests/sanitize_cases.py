@@ -5,7 +5,7 @@ perturbs timing still verifies the numbers.  Not collected by pytest; run as
     compute-sanitizer --tool racecheck python tests/sanitize_cases.py <case> [<case> ...]
 
 Cases: fused_c2 fused_c8 fused_c16 fused_b32 tc_c1 tc_c8 tc_bf16 tc_wide eval_fp32 eval_tf32_h256
-eval_tf32_h1024 eval_bf16 eval_x3 (default: all that the library supports).  Summary: profiles/r02_sanitizer.md."""
+eval_tf32_h1024 eval_bf16 eval_x3 eval_static (default: all that the library supports).  Summary: profiles/r02_sanitizer.md."""
 import os
 import sys
 
@@ -46,12 +46,12 @@ def train_case(hidden, batch, n, cluster, variant, tol, epochs=1):
     return e1, e2
 
 
-def eval_case(hidden, n, variant, tol):
+def eval_case(hidden, n, variant, tol, static=False):
     X, Y = datagen.make_dataset(n, 0.1)
     W1, W2 = O.init_weights(5, 32, hidden)
     B.mlp_init(2, 32, hidden, 1)
     out = torch.zeros(1, dtype=torch.float64, device="cuda")
-    B.mlp_eval_loss_async(dev(X), dev(Y), n, dev(W1), dev(W2), out, variant)
+    (B.mlp_eval_loss_static if static else B.mlp_eval_loss_async)(dev(X), dev(Y), n, dev(W1), dev(W2), out, variant)
     torch.cuda.synchronize()
     lo = O.eval_loss(X, Y, W1, W2)
     e = abs(float(out.item()) - lo) / lo
@@ -76,6 +76,7 @@ CASES = {
     "eval_tf32_h1024": lambda: eval_case(1024, 40000, B.VARIANT_TF32, 5e-3),
     "eval_bf16": lambda: eval_case(256, 40000, B.VARIANT_BF16, 5e-3),
     "eval_x3": lambda: eval_case(256, 40000, B.VARIANT_TF32X3, 1e-5),
+    "eval_static": lambda: eval_case(256, 40000, B.VARIANT_FUSED, 2e-6, static=True),   # scratch in a __device__ array
 }
 
 if __name__ == "__main__":
